@@ -1,0 +1,164 @@
+/* molsim.h — C ABI of the B200-native molecule-agent step engine.
+ *
+ * One handle = one population of molecule agents advanced by hand-written sm_100a CUDA kernels.
+ * The operation is the per-time-step agent update of the simulator of arxiv/paper_2606_14603
+ * (molecules as agents that diffuse, bind by spatial proximity, release
+ * products, cross compartments and are expressed; the per-step update is the
+ * memory-bound hot path that scales linearly with agent count), with the algorithm fixed by
+ * BASELINE.json `north_star` subsystems (1)-(5) and frozen in DESIGN.md §1 ("Step specification").
+ *
+ * Conventions
+ *  - All arithmetic is integer.  Positions are int32 in 0.1 nm units, species uint16
+ *    (0xFFFF = none/DEAD), ids uint32 (DESIGN.md §1 "State").
+ *  - HOST pointers unless a parameter says DEVICE.  The library copies every table it is given;
+ *    the caller keeps ownership of all arguments.  The only device memory the library uses is the
+ *    workspace the caller hands to sim_create (e.g. a torch uint8 tensor) which must outlive the
+ *    handle and must not be touched by the caller meanwhile.
+ *  - All kernels are enqueued on the cudaStream_t given to sim_create.
+ *  - Every function returns SIM_OK (0) or a negative SIM_E_* code; nothing throws or aborts; no
+ *    global state.  A handle is not thread-safe.  There is no CPU fallback: without a CUDA device
+ *    sim_create returns SIM_E_CUDA.
+ */
+#ifndef MOLSIM_H
+#define MOLSIM_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { SIM_OK = 0,
+       SIM_E_INVAL = -1,     /* table validation failed / bad argument (cf. the paper's consistency checker) */
+       SIM_E_CAPACITY = -2,  /* agent slots, counts rows or an output buffer too small */
+       SIM_E_IDSPACE = -3,   /* next_id would pass id_capacity */
+       SIM_E_CUDA = -4 };    /* CUDA runtime error (sim_last_cuda_error has the text) */
+
+/* unimolecular channel kinds — DESIGN.md §1 phase 3 */
+enum { SIM_CH_NONE = 0, SIM_CH_BIRTH = 1, SIM_CH_RELEASE = 2, SIM_CH_CONVERT = 3,
+       SIM_CH_DEGRADE = 4, SIM_CH_DELAYED_BIRTH = 5 };
+/* compartment shapes — DESIGN.md §1 phase 1, reading S1 */
+enum { SIM_SHAPE_CUBE = 0, SIM_SHAPE_SPHERE = 1 };
+
+#define SIM_NONE16 0xFFFFu
+#define SIM_MAX_CHANNELS 4
+#define SIM_MAX_SPECIES 64
+#define SIM_MAX_REACTIONS 64
+#define SIM_MAX_COMPARTMENTS 8
+#define SIM_MAX_RULES 8
+#define SIM_MAX_REPLICAS 64
+
+typedef struct {
+  uint32_t kind;        /* SIM_CH_* */
+  uint32_t thr;         /* fires iff draw < thr (thr = 2^32-1: always); DELAYED_BIRTH: delay in steps >= 1 */
+  uint16_t prod0;       /* species the parent becomes (RELEASE, CONVERT) */
+  uint16_t prod1;       /* species of the newborn (BIRTH, RELEASE, DELAYED_BIRTH) */
+  uint16_t rule;        /* t_first slot (marks_first BIRTH, DELAYED_BIRTH) */
+  uint16_t marks_first; /* BIRTH: firing records t_first[rule] = min(., t) */
+} sim_channel_t;
+
+typedef struct {
+  uint16_t sigma_class; /* row of `tables`; 0 = immobile */
+  uint16_t compartment;
+  uint16_t cross_to;    /* twin species in the adjacent compartment (reading S7) or SIM_NONE16 */
+  uint16_t n_channels;  /* <= SIM_MAX_CHANNELS */
+  uint32_t cross_thr;   /* crossing threshold per membrane contact */
+  sim_channel_t ch[SIM_MAX_CHANNELS];
+} sim_species_t;
+
+/* bimolecular reaction a + b -> cplx: `a` is the anchor that keeps id and position (reading S10) */
+typedef struct { uint16_t a, b, cplx, pad; uint32_t r2 /* units^2 */, thr; } sim_reaction_t;
+
+/* CUBE: lattice 0..L-1 per axis.  SPHERE: |p-c|^2 <= r_out^2 and (r_in < 0 or |p-c|^2 > r_in^2). */
+typedef struct { uint32_t shape; int32_t cx, cy, cz, L, r_out, r_in; } sim_compartment_t;
+
+typedef struct { uint16_t species; uint16_t replica; uint32_t count; } sim_seed_rec_t;
+
+typedef struct {
+  uint32_t n_species, n_reactions, n_compartments, n_sigma_classes;
+  uint32_t table_bits;     /* B: each displacement table has 2^B int16 entries (reading S3) */
+  uint32_t n_rules;        /* t_first slots */
+  uint32_t n_replicas;     /* replica = x >> stride_shift (reading S16); 1 replica: stride_shift = 31 */
+  uint32_t stride_shift;
+  int32_t  extent[3];      /* world bounding box: every valid position has 0 <= p < extent */
+  uint32_t cell_size;      /* spatial-hash cell edge in units, >= max interaction radius; tuning only */
+  uint64_t seed;           /* Philox key of the simulation streams (reading S2) */
+  uint32_t capacity;       /* agent slots (live + dead + newborn of one step) */
+  uint32_t id_capacity;    /* ids ever issued must stay below this */
+  uint32_t counts_rows;    /* rows of the per-step counts log; row t = state after t steps */
+  uint32_t pad;
+  const sim_species_t*     species;       /* [n_species] */
+  const sim_reaction_t*    reactions;     /* [n_reactions] */
+  const sim_compartment_t* compartments;  /* [n_compartments] */
+  const int16_t*           tables;        /* [n_sigma_classes << table_bits], row 0 ignored */
+} sim_config_t;
+
+typedef struct sim sim_t;   /* opaque; owned by the library, freed by sim_destroy */
+
+/* Bytes of DEVICE workspace sim_create needs for this configuration (0 if cfg is invalid). */
+size_t sim_workspace_bytes(const sim_config_t* cfg);
+
+/* Validates the tables (SIM_E_INVAL), copies them to the device, carves the workspace.
+ * d_workspace: DEVICE memory, >= sim_workspace_bytes(cfg), 256-byte aligned, owned by the caller.
+ * cuda_stream: a cudaStream_t (0 = default stream). */
+int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_bytes,
+               void* cuda_stream, sim_t** out);
+
+/* Adds agents: record order gives contiguous fresh ids; positions uniform in the species'
+ * compartment from the PLACE stream keyed by place_seed (DESIGN.md §1 "Seeding", reading S15).
+ * May be called again mid-run (run-time treatment change).  Rewrites counts row t.
+ * Synchronises the stream. */
+int sim_seed_population(sim_t*, const sim_seed_rec_t* recs, uint32_t n_recs, uint64_t place_seed);
+
+/* Advances n_steps time steps (DESIGN.md §1 phases 1-6 per step).  All work is enqueued on the
+ * stream without host synchronisation between steps; the call then waits for the stream once and
+ * returns the sticky device error state (capacity / id space), if any. */
+int sim_step(sim_t*, uint32_t n_steps);
+/* Same, but returns after enqueueing; errors surface at the next synchronising call. */
+int sim_step_async(sim_t*, uint32_t n_steps);
+
+/* Per-step species counts, rows first_row .. first_row+n_rows-1 (row <= steps done):
+ * out[n_rows][n_replicas][n_species], HOST. */
+int sim_read_counts(sim_t*, uint32_t first_row, uint32_t n_rows, uint32_t* out);
+
+/* Live agents sorted by id into HOST arrays of `cap` elements each (any array may be NULL);
+ * *n_out = number of live agents (also set when cap is too small: SIM_E_CAPACITY). */
+int sim_read_agents(sim_t*, uint32_t cap, int32_t* x, int32_t* y, int32_t* z,
+                    uint16_t* species, uint32_t* id, uint32_t* n_out);
+
+/* Replaces the population by explicit agents in any order (checkpoint reload / test hook);
+ * sets the step counter and next_id; rewrites counts row `step`.  HOST arrays. */
+int sim_load_agents(sim_t*, uint32_t n, const int32_t* x, const int32_t* y, const int32_t* z,
+                    const uint16_t* species, const uint32_t* id, uint32_t step, uint32_t next_id);
+
+/* Current scalars (any pointer may be NULL).  Synchronises the stream. */
+int sim_info(sim_t*, uint32_t* n_live, uint32_t* step, uint32_t* next_id, uint32_t* t_first0);
+
+/* Test hook: phase 1 only (move + boundary/compartment rule) on the current state; the step
+ * counter does not advance. */
+int sim_debug_move_only(sim_t*);
+
+/* Number of kernels the handle has launched so far (bench.py's gpu_launches). */
+uint64_t sim_launch_count(const sim_t*);
+
+/* Per-kernel device time: when enabled, every kernel of sim_step is bracketed by CUDA events on
+ * the stream (slower; for bench.py's roofline leg, not for throughput numbers).
+ * sim_kernel_times returns, for each of the SIM_N_KERNELS kernels, accumulated milliseconds and
+ * launch counts since the last enable. */
+#define SIM_N_KERNELS 12
+int sim_profile_enable(sim_t*, int on);
+int sim_kernel_times(sim_t*, float ms[SIM_N_KERNELS], uint32_t launches[SIM_N_KERNELS]);
+const char* sim_kernel_name(int k);
+
+void sim_destroy(sim_t*);
+const char* sim_strerror(int code);
+const char* sim_last_cuda_error(const sim_t*);
+
+/* Test hook: Philox4x32-10 on the device for n (counter,key) pairs; DEVICE pointers
+ * ctr[4n], key[2n], out[4n]; enqueued on `cuda_stream`. */
+int sim_debug_philox(const uint32_t* d_ctr, const uint32_t* d_key, uint32_t* d_out, uint32_t n,
+                     void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

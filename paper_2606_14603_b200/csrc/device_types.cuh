@@ -1,0 +1,111 @@
+// device_types.cuh — device-side tables, launch parameters and small helpers.
+// Product code (CUDA path).  Written from DESIGN.md §1; shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace molsim {
+
+constexpr uint16_t kDead = 0xFFFFu;
+constexpr uint32_t kNever = 0xFFFFFFFFu;
+constexpr uint32_t kNoProp = 0xFFFFFFFFu;
+constexpr int kMaxSpecies = 64;
+constexpr int kMaxReactions = 64;
+constexpr int kMaxCompartments = 8;
+constexpr int kMaxRules = 8;
+
+enum : uint32_t { kTagMove = 1, kTagPair = 2, kTagUni = 3, kTagBirth = 4, kTagPlace = 5 };
+enum : uint8_t { kChNone = 0, kChBirth = 1, kChRelease = 2, kChConvert = 3, kChDegrade = 4, kChDelayed = 5 };
+
+struct DevChannel {
+  uint8_t kind, rule, marks_first, pad;
+  uint16_t prod0, prod1;
+  uint32_t thr;
+};
+struct DevSpecies {
+  uint8_t sigma_class, compartment, n_channels, binds;
+  uint16_t cross_to, pad;
+  uint32_t cross_thr;
+  DevChannel ch[4];
+};
+struct DevComp {
+  int32_t shape, cx, cy, cz, L, r_out, r_in, pad;
+  long long r_out2, r_in2;   // r_in2 = -1 when there is no hole
+};
+struct DevRx { uint16_t a, b, cplx, pad; uint32_t r2, thr; };
+
+struct DevTables {
+  DevSpecies sp[kMaxSpecies];
+  DevComp comp[kMaxCompartments];
+  DevRx rx[kMaxReactions];
+  uint8_t rxmap[kMaxSpecies * kMaxSpecies];   // 0xFF = no reaction
+};
+
+// Scalars that live on the device so that sim_step(n) never needs the host between steps.
+struct Scalars {
+  uint32_t n_slots;        // length of the current (unsorted) arrays, DEAD slots included
+  uint32_t next_id;
+  uint32_t t;              // steps done
+  uint32_t err;            // sticky: bit0 capacity, bit1 id space
+  uint32_t birth_count;    // entries in the birth-parent list of this step
+  uint32_t total_births;   // newborns of this step
+  uint32_t ticket;         // last-block-done counter of the epilogue
+  uint32_t n_read;         // sim_read_agents compaction counter
+  uint32_t t_first[kMaxRules];
+};
+
+// One agent array set (structure of arrays, north_star (1)).
+struct Soa {
+  int32_t* x; int32_t* y; int32_t* z; uint32_t* id;
+};
+
+struct Params {
+  Soa cur, oth;             // cur: state at step start (moved in place); oth: cell-sorted copy
+  uint16_t* sp_cur;         // species of the current state (read by move, written by resolve/births)
+  uint16_t* sp_sorted;      // species in cell-sorted order (written by scatter)
+  uint32_t* off;            // within-cell rank from the histogram pass
+  uint32_t* prop;           // proposal: partner slot (sorted order) or kNoProp
+  uint32_t* cell;           // [n_cells + 1]: counts, then exclusive starts; cell[n_cells] = n_sorted
+  uint32_t* partial;        // scan partials
+  uint32_t* bits;           // birth bitmap, 4 bits per id
+  uint32_t* chunk_prefix;   // exclusive newborn prefix per 64-id chunk
+  uint2* birth_list;        // (parent slot, mask | pre-species << 16)
+  uint32_t* counts;         // [counts_rows][n_replicas][n_species]
+  Scalars* scal;
+  const DevTables* tab;
+  const int16_t* gauss;     // [n_classes << B]
+  uint32_t key0, key1;
+  uint32_t capacity, id_capacity;
+  uint32_t n_species, n_replicas, stride_shift, table_bits, n_classes;
+  int32_t cell_size, cell_shift;   // cell_shift >= 0 when cell_size is a power of two
+  int32_t nx, ny, nz;
+  uint32_t n_cells;
+  int32_t max_r;            // max interaction radius (ceil sqrt of max r2)
+  uint32_t max_r2;
+  uint32_t row_width;       // n_replicas * n_species
+};
+
+__device__ __forceinline__ bool fire(uint32_t u, uint32_t thr) { return thr == 0xFFFFFFFFu || u < thr; }
+
+__device__ __forceinline__ int32_t mirror(int32_t q, int32_t L) {
+  if (q < 0) return -1 - q;
+  if (q >= L) return 2 * L - 1 - q;
+  return q;
+}
+
+__device__ __forceinline__ bool comp_valid(const DevComp& c, int32_t x, int32_t y, int32_t z) {
+  if (c.shape == 0) return x >= 0 && x < c.L && y >= 0 && y < c.L && z >= 0 && z < c.L;
+  long long dx = (long long)x - c.cx, dy = (long long)y - c.cy, dz = (long long)z - c.cz;
+  long long r2 = dx * dx + dy * dy + dz * dz;
+  return r2 <= c.r_out2 && r2 > c.r_in2;
+}
+
+__device__ __forceinline__ int32_t cell_coord(int32_t v, const Params& p) {
+  return p.cell_shift >= 0 ? (v >> p.cell_shift) : (v / p.cell_size);
+}
+__device__ __forceinline__ uint32_t cell_key(int32_t x, int32_t y, int32_t z, const Params& p) {
+  return ((uint32_t)cell_coord(z, p) * (uint32_t)p.ny + (uint32_t)cell_coord(y, p)) * (uint32_t)p.nx +
+         (uint32_t)cell_coord(x, p);
+}
+
+}  // namespace molsim

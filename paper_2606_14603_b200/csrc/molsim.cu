@@ -1,0 +1,556 @@
+// molsim.cu — host side of the C ABI declared in include/molsim.h.
+// Product code (CUDA path): validation, workspace carving, launch sequencing.  Every step of the
+// hot path runs in the kernels of kernels.cuh; there is no CPU fallback.
+#include "../../include/molsim.h"
+#include "kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace molsim;
+
+namespace {
+
+constexpr int kScanBlocks = 592;          // 148 SMs x 4
+constexpr uint32_t kBirthBlocks = 296;    // 148 SMs x 2
+
+enum KernelId { KI_MOVE = 0, KI_CELL_ZERO, KI_CELL_REDUCE, KI_CELL_SCAN, KI_SCATTER, KI_NEIGHBOUR,
+                KI_RESOLVE, KI_BIRTH_REDUCE, KI_BIRTH_SCAN, KI_BIRTHS, KI_EPILOGUE, KI_OTHER };
+const char* kKernelNames[SIM_N_KERNELS] = {
+    "k_move_hist", "memset_cells", "k_cell_reduce", "k_cell_scan", "k_scatter", "k_neighbour",
+    "k_resolve_uni", "k_birth_reduce", "k_birth_scan", "k_births", "k_epilogue", "other"};
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+  size_t soa[2][4], sp_cur, sp_sorted, off, prop, cell, partial, bits, chunk_prefix, birth_list, counts,
+      scal, tab, gauss, total;
+  uint32_t n_cells, nx, ny, nz;
+};
+
+bool make_layout(const sim_config_t* c, Layout& L) {
+  const uint64_t cs = c->cell_size;
+  const uint64_t nx = (c->extent[0] + cs - 1) / cs, ny = (c->extent[1] + cs - 1) / cs, nz = (c->extent[2] + cs - 1) / cs;
+  const uint64_t nc = nx * ny * nz;
+  if (nc == 0 || nc >= 0x7FFFFFF0ull) return false;
+  L.nx = (uint32_t)nx; L.ny = (uint32_t)ny; L.nz = (uint32_t)nz; L.n_cells = (uint32_t)nc;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
+  const size_t cap = c->capacity;
+  for (int b = 0; b < 2; ++b) for (int a = 0; a < 4; ++a) L.soa[b][a] = take(cap * 4);
+  L.sp_cur = take(cap * 2); L.sp_sorted = take(cap * 2);
+  L.off = take(cap * 4); L.prop = take(cap * 4);
+  L.cell = take(((size_t)nc + 1 + 1024) * 4);
+  L.partial = take(4096 * 4);
+  const size_t n_chunks = ((size_t)c->id_capacity + 63) / 64 + 1;
+  L.bits = take(n_chunks * 8 * 4);
+  L.chunk_prefix = take(n_chunks * 4);
+  L.birth_list = take(cap * 8);
+  L.counts = take(((size_t)c->counts_rows + 2) * c->n_replicas * c->n_species * 4);
+  L.scal = take(sizeof(Scalars));
+  L.tab = take(sizeof(DevTables));
+  L.gauss = take(((size_t)c->n_sigma_classes << c->table_bits) * 2);
+  L.total = o;
+  return true;
+}
+
+// Table validation: the in-scope part of the paper's consistency checker plus the
+// bounds the kernels rely on.
+int validate(const sim_config_t* c) {
+  if (!c || !c->species || !c->compartments || !c->tables) return SIM_E_INVAL;
+  if (c->n_reactions && !c->reactions) return SIM_E_INVAL;
+  if (c->n_species == 0 || c->n_species > SIM_MAX_SPECIES || c->n_reactions > SIM_MAX_REACTIONS) return SIM_E_INVAL;
+  if (c->n_compartments == 0 || c->n_compartments > SIM_MAX_COMPARTMENTS || c->n_rules > SIM_MAX_RULES) return SIM_E_INVAL;
+  if (c->table_bits < 1 || c->table_bits > 16 || c->n_sigma_classes < 1 || c->n_sigma_classes > 255) return SIM_E_INVAL;
+  if (c->n_replicas < 1 || c->n_replicas > SIM_MAX_REPLICAS || c->stride_shift > 31) return SIM_E_INVAL;
+  if (c->cell_size == 0 || c->cell_size > 16384) return SIM_E_INVAL;
+  if (c->capacity == 0 || c->capacity > 0x7FFFFFFFu || c->counts_rows == 0 || c->id_capacity == 0) return SIM_E_INVAL;
+  for (int a = 0; a < 3; ++a) if (c->extent[a] <= 0) return SIM_E_INVAL;
+  if (c->n_replicas > 1 && ((uint64_t)c->n_replicas << c->stride_shift) > 0x80000000ull) return SIM_E_INVAL;
+  if ((uint64_t)c->extent[0] > ((uint64_t)c->n_replicas << c->stride_shift)) return SIM_E_INVAL;
+  int32_t max_tab = 0;
+  for (size_t i = (size_t)1 << c->table_bits; i < ((size_t)c->n_sigma_classes << c->table_bits); ++i)
+    max_tab = std::max<int32_t>(max_tab, std::abs((int32_t)c->tables[i]));
+  for (uint32_t i = 0; i < c->n_compartments; ++i) {
+    const sim_compartment_t& k = c->compartments[i];
+    int64_t hi_x;
+    if (k.shape == SIM_SHAPE_CUBE) {
+      if (k.L <= 0 || max_tab >= k.L || k.L > c->extent[1] || k.L > c->extent[2]) return SIM_E_INVAL;
+      hi_x = k.L;
+    } else if (k.shape == SIM_SHAPE_SPHERE) {
+      if (k.r_out <= 0 || k.r_in >= k.r_out) return SIM_E_INVAL;
+      if (k.cx - k.r_out < 0 || k.cy - k.r_out < 0 || k.cz - k.r_out < 0) return SIM_E_INVAL;
+      if ((int64_t)k.cy + k.r_out >= c->extent[1] || (int64_t)k.cz + k.r_out >= c->extent[2]) return SIM_E_INVAL;
+      hi_x = (int64_t)k.cx + k.r_out + 1;
+    } else {
+      return SIM_E_INVAL;
+    }
+    if (c->n_replicas > 1 && hi_x > ((int64_t)1 << c->stride_shift)) return SIM_E_INVAL;
+    if (c->n_replicas == 1 && hi_x > c->extent[0]) return SIM_E_INVAL;
+  }
+  for (uint32_t i = 0; i < c->n_species; ++i) {
+    const sim_species_t& s = c->species[i];
+    if (s.sigma_class >= c->n_sigma_classes || s.compartment >= c->n_compartments) return SIM_E_INVAL;
+    if (s.n_channels > SIM_MAX_CHANNELS) return SIM_E_INVAL;
+    if (s.cross_to != SIM_NONE16) {
+      if (s.cross_to >= c->n_species) return SIM_E_INVAL;
+      const uint32_t oc = c->species[s.cross_to].compartment;
+      if (oc == s.compartment) return SIM_E_INVAL;
+      if (c->compartments[oc].shape == SIM_SHAPE_CUBE || c->compartments[s.compartment].shape == SIM_SHAPE_CUBE)
+        return SIM_E_INVAL;
+    }
+    for (uint32_t k = 0; k < s.n_channels; ++k) {
+      const sim_channel_t& ch = s.ch[k];
+      if (ch.kind > SIM_CH_DELAYED_BIRTH) return SIM_E_INVAL;
+      const bool needs0 = ch.kind == SIM_CH_RELEASE || ch.kind == SIM_CH_CONVERT;
+      const bool needs1 = ch.kind == SIM_CH_RELEASE || ch.kind == SIM_CH_BIRTH || ch.kind == SIM_CH_DELAYED_BIRTH;
+      if (needs0 && (ch.prod0 >= c->n_species || c->species[ch.prod0].compartment != s.compartment)) return SIM_E_INVAL;
+      if (needs1 && (ch.prod1 >= c->n_species || c->species[ch.prod1].compartment != s.compartment)) return SIM_E_INVAL;
+      if ((ch.kind == SIM_CH_DELAYED_BIRTH || ch.marks_first) && ch.rule >= c->n_rules) return SIM_E_INVAL;
+      if (ch.kind == SIM_CH_DELAYED_BIRTH && ch.thr < 1) return SIM_E_INVAL;
+    }
+  }
+  for (uint32_t e = 0; e < c->n_reactions; ++e) {
+    const sim_reaction_t& r = c->reactions[e];
+    if (r.a >= c->n_species || r.b >= c->n_species || r.cplx >= c->n_species) return SIM_E_INVAL;
+    const uint32_t ca = c->species[r.a].compartment;
+    if (c->species[r.b].compartment != ca || c->species[r.cplx].compartment != ca) return SIM_E_INVAL;
+    if ((uint64_t)r.r2 > (uint64_t)c->cell_size * c->cell_size) return SIM_E_INVAL;
+    for (uint32_t f = 0; f < e; ++f) {
+      const sim_reaction_t& q = c->reactions[f];
+      if ((q.a == r.a && q.b == r.b) || (q.a == r.b && q.b == r.a)) return SIM_E_INVAL;
+    }
+  }
+  return SIM_OK;
+}
+
+}  // namespace
+
+struct sim {
+  sim_config_t cfg;
+  Layout lay;
+  Params prm;         // prm.cur / prm.oth always describe the CURRENT parity
+  char* ws = nullptr;
+  cudaStream_t stream = nullptr;
+  uint32_t t_host = 0;           // steps enqueued so far (the host knows t exactly)
+  uint64_t launches = 0;
+  int gauss_in_smem = 0;
+  size_t gauss_bytes = 0;
+  uint32_t grid_agents = 0;
+  uint32_t cell_seg = 0;
+  bool profile = false;
+  float prof_ms[SIM_N_KERNELS] = {};
+  uint32_t prof_n[SIM_N_KERNELS] = {};
+  std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> prof_pending;
+  std::string cuda_err;
+  int sticky = SIM_OK;
+
+  int cuda_fail(cudaError_t e, const char* where) {
+    cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
+    return SIM_E_CUDA;
+  }
+};
+
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return s->cuda_fail(e_, #call); } while (0)
+
+namespace {
+
+struct ProfScope {
+  sim* s; int k; cudaEvent_t a = nullptr, b = nullptr;
+  ProfScope(sim* s_, int k_) : s(s_), k(k_) {
+    if (s->profile) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, s->stream); }
+  }
+  ~ProfScope() {
+    s->launches++;
+    if (s->profile) { cudaEventRecord(b, s->stream); s->prof_pending.push_back({k, {a, b}}); }
+  }
+};
+
+void prof_collect(sim* s) {
+  for (auto& pe : s->prof_pending) {
+    float ms = 0.f;
+    cudaEventSynchronize(pe.second.second);
+    cudaEventElapsedTime(&ms, pe.second.first, pe.second.second);
+    s->prof_ms[pe.first] += ms; s->prof_n[pe.first]++;
+    cudaEventDestroy(pe.second.first); cudaEventDestroy(pe.second.second);
+  }
+  s->prof_pending.clear();
+}
+
+int read_scalars(sim* s, Scalars* out) {
+  CK(cudaMemcpyAsync(out, s->prm.scal, sizeof(Scalars), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return SIM_OK;
+}
+
+int err_from_bits(uint32_t bits) {
+  if (bits & 1u) return SIM_E_CAPACITY;
+  if (bits & 2u) return SIM_E_IDSPACE;
+  return SIM_OK;
+}
+
+// counts row r <- histogram of the current state; row r+1 <- copy (base of the next step's deltas)
+int recount_row(sim* s, uint32_t r, uint32_t n_slots) {
+  CK(cudaMemsetAsync(s->prm.counts + (size_t)r * s->prm.row_width, 0, (size_t)s->prm.row_width * 4, s->stream));
+  if (n_slots) {
+    ProfScope ps(s, KI_OTHER);
+    k_count_row<<<std::min<uint32_t>((n_slots + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, r, n_slots);
+  }
+  { ProfScope ps(s, KI_OTHER); k_copy_row<<<1, 256, 0, s->stream>>>(s->prm, r); }
+  CK(cudaGetLastError());
+  return SIM_OK;
+}
+
+int enqueue_step(sim* s) {
+  Params& p = s->prm;
+  const uint32_t ga = s->grid_agents;
+  {
+    ProfScope ps(s, KI_CELL_ZERO);
+    CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->stream));
+  }
+  { ProfScope ps(s, KI_MOVE);
+    k_move_hist<true><<<ga, 256, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(p, s->gauss_in_smem); }
+  { ProfScope ps(s, KI_CELL_REDUCE);
+    k_cell_reduce<<<kScanBlocks, kScanThreads, 0, s->stream>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+  { ProfScope ps(s, KI_CELL_SCAN);
+    k_cell_scan<<<kScanBlocks, kScanThreads, 0, s->stream>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+  { ProfScope ps(s, KI_SCATTER); k_scatter<<<ga, 256, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_NEIGHBOUR); k_neighbour<<<ga * 2, 128, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_RESOLVE); k_resolve_uni<<<ga, 256, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_BIRTH_REDUCE); k_birth_reduce<<<kBirthBlocks, kScanThreads, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_BIRTH_SCAN); k_birth_scan<<<kBirthBlocks, kScanThreads, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_BIRTHS); k_births<<<148, 128, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_EPILOGUE); k_epilogue<<<148, 256, 0, s->stream>>>(p); }
+  CK(cudaGetLastError());
+  std::swap(p.cur, p.oth);   // the sorted copy (+ newborns) is the next step's current state
+  s->t_host++;
+  return SIM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t sim_workspace_bytes(const sim_config_t* cfg) {
+  Layout L;
+  if (validate(cfg) != SIM_OK || !make_layout(cfg, L)) return 0;
+  return L.total;
+}
+
+int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_bytes, void* cuda_stream, sim_t** out) {
+  if (!out) return SIM_E_INVAL;
+  *out = nullptr;
+  int v = validate(cfg);
+  if (v) return v;
+  Layout L;
+  if (!make_layout(cfg, L)) return SIM_E_INVAL;
+  if (!d_workspace || workspace_bytes < L.total || ((uintptr_t)d_workspace & 255u)) return SIM_E_INVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return SIM_E_CUDA;
+
+  sim* s = new sim();
+  s->cfg = *cfg;
+  s->cfg.species = nullptr; s->cfg.reactions = nullptr; s->cfg.compartments = nullptr; s->cfg.tables = nullptr;
+  s->lay = L;
+  s->ws = (char*)d_workspace;
+  s->stream = (cudaStream_t)cuda_stream;
+
+  // host image of the device tables
+  std::vector<DevTables> tabv(1);
+  DevTables& T = tabv[0];
+  std::memset(&T, 0, sizeof(T));
+  std::memset(T.rxmap, 0xFF, sizeof(T.rxmap));
+  uint32_t max_r2 = 0;
+  for (uint32_t e = 0; e < cfg->n_reactions; ++e) {
+    const sim_reaction_t& r = cfg->reactions[e];
+    T.rx[e] = DevRx{r.a, r.b, r.cplx, 0, r.r2, r.thr};
+    T.rxmap[r.a * kMaxSpecies + r.b] = (uint8_t)e;
+    T.rxmap[r.b * kMaxSpecies + r.a] = (uint8_t)e;
+    max_r2 = std::max(max_r2, r.r2);
+  }
+  for (uint32_t i = 0; i < cfg->n_species; ++i) {
+    const sim_species_t& a = cfg->species[i];
+    DevSpecies& d = T.sp[i];
+    d.sigma_class = (uint8_t)a.sigma_class; d.compartment = (uint8_t)a.compartment;
+    d.n_channels = (uint8_t)a.n_channels; d.cross_to = a.cross_to; d.cross_thr = a.cross_thr;
+    d.binds = 0;
+    for (uint32_t e = 0; e < cfg->n_reactions; ++e)
+      if (cfg->reactions[e].a == i || cfg->reactions[e].b == i) d.binds = 1;
+    for (uint32_t k = 0; k < a.n_channels; ++k) {
+      const sim_channel_t& c = a.ch[k];
+      d.ch[k] = DevChannel{(uint8_t)c.kind, (uint8_t)c.rule, (uint8_t)(c.marks_first ? 1 : 0), 0, c.prod0, c.prod1, c.thr};
+    }
+  }
+  for (uint32_t i = 0; i < cfg->n_compartments; ++i) {
+    const sim_compartment_t& a = cfg->compartments[i];
+    DevComp& d = T.comp[i];
+    d.shape = (int32_t)a.shape; d.cx = a.cx; d.cy = a.cy; d.cz = a.cz; d.L = a.L; d.r_out = a.r_out; d.r_in = a.r_in;
+    d.r_out2 = (long long)a.r_out * a.r_out;
+    d.r_in2 = a.r_in < 0 ? -1ll : (long long)a.r_in * a.r_in;
+  }
+
+  Params& p = s->prm;
+  std::memset(&p, 0, sizeof(p));
+  char* w = s->ws;
+  auto soa = [&](int b) { return Soa{(int32_t*)(w + L.soa[b][0]), (int32_t*)(w + L.soa[b][1]),
+                                     (int32_t*)(w + L.soa[b][2]), (uint32_t*)(w + L.soa[b][3])}; };
+  p.cur = soa(0); p.oth = soa(1);
+  p.sp_cur = (uint16_t*)(w + L.sp_cur); p.sp_sorted = (uint16_t*)(w + L.sp_sorted);
+  p.off = (uint32_t*)(w + L.off); p.prop = (uint32_t*)(w + L.prop);
+  p.cell = (uint32_t*)(w + L.cell); p.partial = (uint32_t*)(w + L.partial);
+  p.bits = (uint32_t*)(w + L.bits); p.chunk_prefix = (uint32_t*)(w + L.chunk_prefix);
+  p.birth_list = (uint2*)(w + L.birth_list); p.counts = (uint32_t*)(w + L.counts);
+  p.scal = (Scalars*)(w + L.scal); p.tab = (const DevTables*)(w + L.tab); p.gauss = (const int16_t*)(w + L.gauss);
+  p.key0 = (uint32_t)cfg->seed; p.key1 = (uint32_t)(cfg->seed >> 32);
+  p.capacity = cfg->capacity; p.id_capacity = cfg->id_capacity;
+  p.n_species = cfg->n_species; p.n_replicas = cfg->n_replicas; p.stride_shift = cfg->stride_shift;
+  p.table_bits = cfg->table_bits; p.n_classes = cfg->n_sigma_classes;
+  p.cell_size = (int32_t)cfg->cell_size;
+  p.cell_shift = -1;
+  for (int b = 0; b < 31; ++b) if ((1u << b) == cfg->cell_size) p.cell_shift = b;
+  p.nx = (int32_t)L.nx; p.ny = (int32_t)L.ny; p.nz = (int32_t)L.nz; p.n_cells = L.n_cells;
+  p.max_r2 = max_r2;
+  p.max_r = (int32_t)std::ceil(std::sqrt((double)max_r2));
+  while ((uint64_t)p.max_r * p.max_r < max_r2) p.max_r++;
+  p.row_width = cfg->n_replicas * cfg->n_species;
+
+  s->gauss_bytes = ((size_t)cfg->n_sigma_classes << cfg->table_bits) * 2;
+  s->gauss_in_smem = s->gauss_bytes <= 160 * 1024;
+  s->grid_agents = (uint32_t)std::min<uint64_t>(((uint64_t)cfg->capacity + 255) / 256, 148ull * 8);
+  s->cell_seg = (uint32_t)align_up(((size_t)L.n_cells + kScanBlocks - 1) / kScanBlocks, 1024);
+
+  cudaError_t e;
+  if (s->gauss_in_smem && s->gauss_bytes > 48 * 1024) {
+    e = cudaFuncSetAttribute(k_move_hist<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->gauss_bytes);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_move_hist<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->gauss_bytes);
+    if (e != cudaSuccess) { delete s; return SIM_E_CUDA; }
+  }
+  Scalars sc;
+  std::memset(&sc, 0, sizeof(sc));
+  for (int r = 0; r < kMaxRules; ++r) sc.t_first[r] = kNever;
+  bool ok = true;
+  ok = ok && cudaMemsetAsync(p.bits, 0, L.chunk_prefix - L.bits, s->stream) == cudaSuccess;
+  ok = ok && cudaMemsetAsync(p.counts, 0, L.scal - L.counts, s->stream) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(p.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync((void*)p.tab, &T, sizeof(T), cudaMemcpyHostToDevice, s->stream) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync((void*)p.gauss, cfg->tables, s->gauss_bytes, cudaMemcpyHostToDevice, s->stream) == cudaSuccess;
+  ok = ok && cudaStreamSynchronize(s->stream) == cudaSuccess;
+  if (!ok) { delete s; return SIM_E_CUDA; }
+  *out = s;
+  return SIM_OK;
+}
+
+void sim_destroy(sim_t* s) {
+  if (!s) return;
+  cudaStreamSynchronize(s->stream);
+  prof_collect(s);
+  delete s;
+}
+
+int sim_seed_population(sim_t* s, const sim_seed_rec_t* recs, uint32_t n_recs, uint64_t place_seed) {
+  if (!s || (!recs && n_recs)) return SIM_E_INVAL;
+  uint64_t total = 0;
+  for (uint32_t i = 0; i < n_recs; ++i) {
+    if (recs[i].species >= s->cfg.n_species || recs[i].replica >= s->cfg.n_replicas) return SIM_E_INVAL;
+    total += recs[i].count;
+  }
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  if (sc.err) return err_from_bits(sc.err);
+  if ((uint64_t)sc.n_slots + total > s->cfg.capacity) return SIM_E_CAPACITY;
+  if ((uint64_t)sc.next_id + total > s->cfg.id_capacity) return SIM_E_IDSPACE;
+  uint32_t dst = sc.n_slots, id = sc.next_id;
+  for (uint32_t i = 0; i < n_recs; ++i) {
+    if (!recs[i].count) continue;
+    ProfScope ps(s, KI_OTHER);
+    k_seed<<<std::min<uint32_t>((recs[i].count + 255) / 256, 148 * 8), 256, 0, s->stream>>>(
+        s->prm, recs[i].species, recs[i].replica, recs[i].count, id, dst, (uint32_t)place_seed, (uint32_t)(place_seed >> 32));
+    dst += recs[i].count; id += recs[i].count;
+  }
+  CK(cudaGetLastError());
+  sc.n_slots = dst; sc.next_id = id;
+  CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
+  r = recount_row(s, sc.t, sc.n_slots);
+  if (r) return r;
+  CK(cudaStreamSynchronize(s->stream));
+  return SIM_OK;
+}
+
+int sim_step_async(sim_t* s, uint32_t n_steps) {
+  if (!s) return SIM_E_INVAL;
+  if (s->sticky) return s->sticky;
+  if ((uint64_t)s->t_host + n_steps >= s->cfg.counts_rows) return SIM_E_CAPACITY;
+  for (uint32_t i = 0; i < n_steps; ++i) {
+    int r = enqueue_step(s);
+    if (r) return r;
+  }
+  return SIM_OK;
+}
+
+int sim_step(sim_t* s, uint32_t n_steps) {
+  int r = sim_step_async(s, n_steps);
+  if (r) return r;
+  uint32_t err = 0;
+  CK(cudaMemcpyAsync(&err, &s->prm.scal->err, 4, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  if (s->profile) prof_collect(s);
+  if (err) { s->sticky = err_from_bits(err); return s->sticky; }
+  return SIM_OK;
+}
+
+int sim_read_counts(sim_t* s, uint32_t first_row, uint32_t n_rows, uint32_t* out) {
+  if (!s || !out || (uint64_t)first_row + n_rows > (uint64_t)s->t_host + 1) return SIM_E_INVAL;
+  CK(cudaMemcpyAsync(out, s->prm.counts + (size_t)first_row * s->prm.row_width,
+                     (size_t)n_rows * s->prm.row_width * 4, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return SIM_OK;
+}
+
+int sim_info(sim_t* s, uint32_t* n_live, uint32_t* step, uint32_t* next_id, uint32_t* t_first0) {
+  if (!s) return SIM_E_INVAL;
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  if (n_live) {
+    std::vector<uint32_t> row(s->prm.row_width);
+    CK(cudaMemcpy(row.data(), s->prm.counts + (size_t)sc.t * s->prm.row_width, row.size() * 4, cudaMemcpyDeviceToHost));
+    uint64_t tot = 0;
+    for (uint32_t v : row) tot += v;
+    *n_live = (uint32_t)tot;
+  }
+  if (step) *step = sc.t;
+  if (next_id) *next_id = sc.next_id;
+  if (t_first0) *t_first0 = sc.t_first[0];
+  return SIM_OK;
+}
+
+int sim_read_agents(sim_t* s, uint32_t cap, int32_t* x, int32_t* y, int32_t* z, uint16_t* species, uint32_t* id,
+                    uint32_t* n_out) {
+  if (!s || !n_out) return SIM_E_INVAL;
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  CK(cudaMemsetAsync(&s->prm.scal->n_read, 0, 4, s->stream));
+  if (sc.n_slots) {
+    ProfScope ps(s, KI_OTHER);
+    k_gather_live<<<std::min<uint32_t>((sc.n_slots + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, sc.n_slots);
+  }
+  CK(cudaGetLastError());
+  uint32_t n = 0;
+  CK(cudaMemcpyAsync(&n, &s->prm.scal->n_read, 4, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  *n_out = n;
+  if (n > cap) return SIM_E_CAPACITY;
+  if (n == 0) return SIM_OK;
+  std::vector<uint32_t> hid(n);
+  CK(cudaMemcpy(hid.data(), s->prm.oth.id, (size_t)n * 4, cudaMemcpyDeviceToHost));
+  // id-sorted order: ids are unique and < next_id, so one pass over the id space sorts them
+  std::vector<uint32_t> where((size_t)sc.next_id, 0xFFFFFFFFu), order;
+  order.reserve(n);
+  for (uint32_t i = 0; i < n; ++i) where[hid[i]] = i;
+  for (uint32_t v = 0; v < sc.next_id; ++v) if (where[v] != 0xFFFFFFFFu) order.push_back(where[v]);
+  if (order.size() != n) return SIM_E_INVAL;   // duplicate ids: internal error
+  std::vector<int32_t> tmp(n);
+  const int32_t* srcs[3] = {s->prm.oth.x, s->prm.oth.y, s->prm.oth.z};
+  int32_t* dsts[3] = {x, y, z};
+  for (int a = 0; a < 3; ++a) {
+    if (!dsts[a]) continue;
+    CK(cudaMemcpy(tmp.data(), srcs[a], (size_t)n * 4, cudaMemcpyDeviceToHost));
+    for (uint32_t i = 0; i < n; ++i) dsts[a][i] = tmp[order[i]];
+  }
+  if (species) {
+    std::vector<uint16_t> ts(n);
+    CK(cudaMemcpy(ts.data(), s->prm.sp_sorted, (size_t)n * 2, cudaMemcpyDeviceToHost));
+    for (uint32_t i = 0; i < n; ++i) species[i] = ts[order[i]];
+  }
+  if (id) for (uint32_t i = 0; i < n; ++i) id[i] = hid[order[i]];
+  return SIM_OK;
+}
+
+int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, const int32_t* z,
+                    const uint16_t* species, const uint32_t* id, uint32_t step, uint32_t next_id) {
+  if (!s || n > s->cfg.capacity || (uint64_t)step + 1 > s->cfg.counts_rows || next_id > s->cfg.id_capacity)
+    return SIM_E_INVAL;
+  if (n && (!x || !y || !z || !species || !id)) return SIM_E_INVAL;
+  for (uint32_t i = 0; i < n; ++i) if (species[i] >= s->cfg.n_species || id[i] >= next_id) return SIM_E_INVAL;
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  CK(cudaMemcpyAsync(s->prm.cur.x, x, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->prm.cur.y, y, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->prm.cur.z, z, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->prm.cur.id, id, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->prm.sp_cur, species, (size_t)n * 2, cudaMemcpyHostToDevice, s->stream));
+  sc.n_slots = n; sc.next_id = next_id; sc.t = step; sc.err = 0;
+  sc.birth_count = sc.total_births = sc.ticket = 0;
+  CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
+  s->t_host = step; s->sticky = SIM_OK;
+  r = recount_row(s, step, n);
+  if (r) return r;
+  CK(cudaStreamSynchronize(s->stream));
+  return SIM_OK;
+}
+
+int sim_debug_move_only(sim_t* s) {
+  if (!s) return SIM_E_INVAL;
+  { ProfScope ps(s, KI_MOVE);
+    k_move_hist<false><<<s->grid_agents, 256, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(s->prm, s->gauss_in_smem); }
+  CK(cudaGetLastError());
+  // crossing deltas went to row t+1: fold them back so that row t describes the moved state
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  r = recount_row(s, sc.t, sc.n_slots);
+  if (r) return r;
+  CK(cudaStreamSynchronize(s->stream));
+  return SIM_OK;
+}
+
+uint64_t sim_launch_count(const sim_t* s) { return s ? s->launches : 0; }
+
+int sim_profile_enable(sim_t* s, int on) {
+  if (!s) return SIM_E_INVAL;
+  cudaStreamSynchronize(s->stream);
+  prof_collect(s);
+  s->profile = on != 0;
+  std::memset(s->prof_ms, 0, sizeof(s->prof_ms));
+  std::memset(s->prof_n, 0, sizeof(s->prof_n));
+  return SIM_OK;
+}
+
+int sim_kernel_times(sim_t* s, float ms[SIM_N_KERNELS], uint32_t launches[SIM_N_KERNELS]) {
+  if (!s) return SIM_E_INVAL;
+  cudaStreamSynchronize(s->stream);
+  prof_collect(s);
+  for (int k = 0; k < SIM_N_KERNELS; ++k) { if (ms) ms[k] = s->prof_ms[k]; if (launches) launches[k] = s->prof_n[k]; }
+  return SIM_OK;
+}
+
+const char* sim_kernel_name(int k) { return (k >= 0 && k < SIM_N_KERNELS) ? kKernelNames[k] : ""; }
+
+const char* sim_strerror(int code) {
+  switch (code) {
+    case SIM_OK: return "ok";
+    case SIM_E_INVAL: return "invalid argument or table validation failed";
+    case SIM_E_CAPACITY: return "capacity exceeded (agent slots, counts rows or output buffer)";
+    case SIM_E_IDSPACE: return "id space exhausted";
+    case SIM_E_CUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+
+const char* sim_last_cuda_error(const sim_t* s) { return s ? s->cuda_err.c_str() : ""; }
+
+int sim_debug_philox(const uint32_t* d_ctr, const uint32_t* d_key, uint32_t* d_out, uint32_t n, void* cuda_stream) {
+  if (!d_ctr || !d_key || !d_out) return SIM_E_INVAL;
+  if (n) k_debug_philox<<<(n + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(d_ctr, d_key, d_out, n);
+  return cudaGetLastError() == cudaSuccess ? SIM_OK : SIM_E_CUDA;
+}
+
+}  // extern "C"
