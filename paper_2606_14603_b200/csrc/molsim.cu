@@ -160,12 +160,12 @@ struct sim {
 namespace {
 
 struct ProfScope {
-  sim* s; int k; cudaEvent_t a = nullptr, b = nullptr;
-  ProfScope(sim* s_, int k_) : s(s_), k(k_) {
+  sim* s; int k; bool is_kernel; cudaEvent_t a = nullptr, b = nullptr;
+  ProfScope(sim* s_, int k_, bool is_kernel_ = true) : s(s_), k(k_), is_kernel(is_kernel_) {
     if (s->profile) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, s->stream); }
   }
   ~ProfScope() {
-    s->launches++;
+    if (is_kernel) s->launches++;   // memsets are not kernels of ours
     if (s->profile) { cudaEventRecord(b, s->stream); s->prof_pending.push_back({k, {a, b}}); }
   }
 };
@@ -209,7 +209,7 @@ int enqueue_step(sim* s) {
   Params& p = s->prm;
   const uint32_t ga = s->grid_agents;
   {
-    ProfScope ps(s, KI_CELL_ZERO);
+    ProfScope ps(s, KI_CELL_ZERO, false);
     CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->stream));
   }
   { ProfScope ps(s, KI_MOVE);
