@@ -111,13 +111,30 @@ def measured_peak():
 
 
 def ledger_bytes_per_agent(kernel, c):
-    """Algorithmic HBM bytes per live agent per launch; c = cells per agent."""
+    """Algorithmic HBM bytes per live agent per launch: SURVEY.md §8(d) "Design B" column, kernel by
+    kernel (DESIGN.md §5 maps each of our kernels to its row); c = cells per agent."""
+    return {
+        "k_move_hist": 18 + 12 + 8 * c,          # K1: R soa, W xyz, cell count RMW
+        "memset_cells": 0.0, "k_cell_reduce": 0.0,
+        "k_cell_scan": 8 * c,                    # K2
+        "k_scatter": 18 + 18 + 8 * c,            # K3: R soa, W soa, cell starts
+        "k_pairs": 18 + 4 + 8 * c,               # K4: R soa, W proposal, cell starts
+        "k_resolve": 0.0,
+        "k_uni": 14 + 4,                         # K5: resolve + unimolecular
+        "k_births": 0.5,                         # K6: births only + id bitmap
+    }.get(kernel, 0.0)
+
+
+def moved_bytes_per_agent(kernel, c):
+    """What THIS implementation must move per live agent per launch: smaller than the
+    §8(d) ledger where a pass was elided (sparse proposals), larger where it keeps an extra array (off)."""
     return {
         "k_move_hist": 18 + 12 + 4 + 8 * c,      # R soa, W xyz, W off, cell count RMW
-        "k_scatter": 18 + 4 + 18 + 4 * c,        # R soa + off, W soa, R cell starts
-        "k_neighbour": 18 + 4 + 4 * c,           # R soa, W proposal, R cell starts
-        "k_resolve_uni": 2 + 4 + 4 + 2,          # R species, id, proposal; W species
         "memset_cells": 4 * c, "k_cell_reduce": 4 * c, "k_cell_scan": 8 * c,
+        "k_scatter": 18 + 4 + 18 + 4 * c,        # R soa + off, W soa, R cell starts
+        "k_pairs": 14 + 0.125 + 4 * c,           # R xyz + species, W 1 bit; R cell starts
+        "k_resolve": 0.125,                      # R proposal bitmap
+        "k_uni": 2,                              # R species (id / position only where a channel exists)
     }.get(kernel, 0.0)
 
 
@@ -258,9 +275,12 @@ def run_gpu(args):
         except Exception:
             traffic = None
     step_bytes = sum(ledger_bytes_per_agent(k, c_per_agent) for k in step_kernels) * n_live_mean
+    moved_bytes = sum(moved_bytes_per_agent(k, c_per_agent) for k in step_kernels) * n_live_mean
     per_kernel = {k: {"ms": round(v[0] / v[1], 4), "share": round(v[0] / tot_ms, 4),
                       "ledger_gbs": round(ledger_bytes_per_agent(k, n_cells / n_live_prof) * n_live_prof /
-                                          (v[0] / v[1] * 1e-3) / 1e9, 1)}
+                                          (v[0] / v[1] * 1e-3) / 1e9, 1),
+                      "moved_gbs": round(moved_bytes_per_agent(k, n_cells / n_live_prof) * n_live_prof /
+                                         (v[0] / v[1] * 1e-3) / 1e9, 1)}
                   for k, v in step_kernels.items()}
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the state, one step, D2H of the counts row
@@ -315,7 +335,8 @@ def run_gpu(args):
                    "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)",
                    "l2": "inputs larger than L2 (SoA ping-pong %.0f MB vs 126 MB L2), no flush" %
                          (2 * BYTES_PER_AGENT * n_live_mean / 1e6),
-                   "bytes_per_agent_step_ledger": round(step_bytes / n_live_mean, 1)},
+                   "bytes_per_agent_step_ledger": round(step_bytes / n_live_mean, 1),
+                   "bytes_per_agent_step_moved": round(moved_bytes / n_live_mean, 1)},
         "clocks": clocks,
         "e2e": {"value": e2e_agent_steps / e2e_dt, "unit": UNIT,
                 "h2d_bytes_per_step": BYTES_PER_AGENT * n_host, "d2h_bytes_per_step": int(row.nbytes),
@@ -327,7 +348,8 @@ def run_gpu(args):
                      "kernel_ms": dom_ms, "kernel_share_of_step": step_kernels[dom][0] / tot_ms,
                      "whole_step": {"achieved": step_bytes / (ms / K * 1e-3) / 1e9,
                                     "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
-                                    "frac_of_8TBs_nominal": step_bytes / (ms / K * 1e-3) / 1e9 / 8000.0},
+                                    "frac_of_8TBs_nominal": step_bytes / (ms / K * 1e-3) / 1e9 / 8000.0,
+                                    "moved_gbs": moved_bytes / (ms / K * 1e-3) / 1e9},
                      "per_kernel": per_kernel},
     }
     if world == 1 and not args.no_cpu:

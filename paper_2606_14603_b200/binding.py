@@ -8,7 +8,7 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmolsim.so")
-N_KERNELS = 12
+N_KERNELS = 13
 E_INVAL, E_CAPACITY, E_IDSPACE, E_CUDA = -1, -2, -3, -4
 
 

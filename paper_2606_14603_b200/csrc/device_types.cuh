@@ -56,15 +56,15 @@ struct Scalars {
 
 // One agent array set (structure of arrays, north_star (1)).
 struct Soa {
-  int32_t* x; int32_t* y; int32_t* z; uint32_t* id;
+  int32_t* x; int32_t* y; int32_t* z; uint32_t* id; uint16_t* sp;
 };
 
 struct Params {
-  Soa cur, oth;             // cur: state at step start (moved in place); oth: cell-sorted copy
-  uint16_t* sp_cur;         // species of the current state (read by move, written by resolve/births)
-  uint16_t* sp_sorted;      // species in cell-sorted order (written by scatter)
+  Soa cur, oth;             // cur: state at step start (moved in place); oth: cell-sorted copy,
+                            // on which bind / unimolecular / births act in place
   uint32_t* off;            // within-cell rank from the histogram pass
-  uint32_t* prop;           // proposal: partner slot (sorted order) or kNoProp
+  uint32_t* prop;           // proposal: partner slot (sorted order); valid only where hasprop is set
+  uint32_t* hasprop;        // 1 bit per sorted slot: the agent proposed this step (rewritten every step)
   uint32_t* cell;           // [n_cells + 1]: counts, then exclusive starts; cell[n_cells] = n_sorted
   uint32_t* partial;        // scan partials
   uint32_t* bits;           // birth bitmap, 4 bits per id
@@ -77,12 +77,15 @@ struct Params {
   uint32_t key0, key1;
   uint32_t capacity, id_capacity;
   uint32_t n_species, n_replicas, stride_shift, table_bits, n_classes;
-  int32_t cell_size, cell_shift;   // cell_shift >= 0 when cell_size is a power of two
+  int32_t cell_size;
+  uint32_t cell_magic, cell_mshift;   // v / cell_size == umulhi(v, cell_magic) >> cell_mshift for 0 <= v < 2^31
   int32_t nx, ny, nz;
   uint32_t n_cells;
   int32_t max_r;            // max interaction radius (ceil sqrt of max r2)
   uint32_t max_r2;
   uint32_t row_width;       // n_replicas * n_species
+  unsigned long long binds_mask;   // bit s: species s takes part in a bimolecular reaction
+  unsigned long long chan_mask;    // bit s: species s has unimolecular channels
 };
 
 __device__ __forceinline__ bool fire(uint32_t u, uint32_t thr) { return thr == 0xFFFFFFFFu || u < thr; }
@@ -100,8 +103,11 @@ __device__ __forceinline__ bool comp_valid(const DevComp& c, int32_t x, int32_t 
   return r2 <= c.r_out2 && r2 > c.r_in2;
 }
 
+// Exact floor(v / cell_size) for 0 <= v < 2^31 by multiply-high: with l = ceil(log2 d),
+// m = floor(2^(31+l) / d) + 1 satisfies 2^(31+l) < m d <= 2^(31+l) + 2^l (Granlund-Montgomery, N = 31),
+// so v / d = (v m) >> (31 + l); d >= 2 gives l >= 1 and m < 2^32, hence umulhi and a shift by l - 1.
 __device__ __forceinline__ int32_t cell_coord(int32_t v, const Params& p) {
-  return p.cell_shift >= 0 ? (v >> p.cell_shift) : (v / p.cell_size);
+  return (int32_t)(__umulhi((uint32_t)v, p.cell_magic) >> p.cell_mshift);
 }
 __device__ __forceinline__ uint32_t cell_key(int32_t x, int32_t y, int32_t z, const Params& p) {
   return ((uint32_t)cell_coord(z, p) * (uint32_t)p.ny + (uint32_t)cell_coord(y, p)) * (uint32_t)p.nx +

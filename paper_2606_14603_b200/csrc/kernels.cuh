@@ -1,8 +1,8 @@
 // kernels.cuh — the hand-written sm_100a kernels of the molecule-agent step.
 // Product code (CUDA path).  Shares nothing with oracle/.
 //
-// One step = K1 move+hist -> K2 cell scan (2 launches) -> K3 scatter -> K4 neighbour/proposal ->
-// K5 resolve+unimolecular -> K6 birth scan (2 launches) + birth placement -> K7 epilogue.
+// One step = K1 move+hist -> K2 cell scan (2 launches) -> K3 scatter -> K4 pair search/proposal ->
+// K4b resolve -> K5 unimolecular -> K6 birth scan (2 launches) + birth placement -> K7 epilogue.
 // Every decision is keyed by agent id (never by slot), so the nondeterministic slot order the
 // histogram atomics produce inside a cell cannot change any result.
 #pragma once
@@ -71,11 +71,17 @@ __device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* s_warp /*[9]
 // ----------------------------------------------------------------------------- K1 move + histogram
 // Phase 1 (Brownian move, boundary and compartment rule) fused with the cell-key histogram of the
 // counting sort.  Gaussian inverse-CDF tables are staged in shared memory.
-// The histogram uses warp-aggregated atomics (__match_any_sync on the cell key): agents are
-// nearly cell-sorted from the previous step, so a warp touches few distinct cells.
-// Counts deltas for membrane crossings go straight to counts row t+1 (rare events).
+// A block walks tiles of 256 x kMoveUnroll agents; every thread keeps kMoveUnroll agents in flight
+// (all loads issued before the first Philox, all histogram atomics before the first rank store) so
+// that HBM and L2-atomic latency overlap.  The histogram uses warp-aggregated atomics
+// (__match_any_sync on the cell key): agents arrive nearly cell-sorted from the previous step, so a
+// warp touches few distinct cells.  Counts deltas for membrane crossings go straight to counts
+// row t+1 (rare events).
+constexpr int kMoveUnroll = 4;
+constexpr int kMoveThreads = 256;
+
 template <bool kHist>
-__global__ void __launch_bounds__(256) k_move_hist(Params p, int gauss_in_smem) {
+__global__ void __launch_bounds__(kMoveThreads) k_move_hist(Params p, int gauss_in_smem) {
   extern __shared__ int16_t s_gauss[];
   const int16_t* g = p.gauss;
   if (gauss_in_smem) {
@@ -89,55 +95,71 @@ __global__ void __launch_bounds__(256) k_move_hist(Params p, int gauss_in_smem) 
   const uint32_t sh = 32u - p.table_bits;
   const uint32_t lane = threadIdx.x & 31u;
   uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
-  const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t base = blockIdx.x * blockDim.x; base < n; base += stride) {   // warp-uniform trip count
-    const uint32_t i = base + threadIdx.x;
-    uint32_t key = 0xFFFFFFFFu;
-    bool live = false;
-    if (i < n) {
-      uint16_t s = p.sp_cur[i];
-      if (s != kDead) {
-        live = true;
-        int32_t x = p.cur.x[i], y = p.cur.y[i], z = p.cur.z[i];
-        const DevSpecies& S = T->sp[s];
-        const uint32_t cls = S.sigma_class;
-        if (cls) {
-          const uint32_t id = p.cur.id[i];
-          const uint4 r = philox4x32_10(id, 0u, t, kTagMove, p.key0, p.key1);
-          const int16_t* tb = g + (cls << p.table_bits);
-          const int32_t rbase = (int32_t)(((uint32_t)x >> p.stride_shift) << p.stride_shift);
-          int32_t qx = x - rbase + tb[r.x >> sh], qy = y + tb[r.y >> sh], qz = z + tb[r.z >> sh];
-          const DevComp& c = T->comp[S.compartment];
-          bool accept = true;
-          if (c.shape == 0) {
-            qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L);
-          } else if (!comp_valid(c, qx, qy, qz)) {
-            accept = false;
-            const uint16_t ct = S.cross_to;
-            if (ct != kDead && comp_valid(T->comp[T->sp[ct].compartment], qx, qy, qz) && fire(r.w, S.cross_thr)) {
-              accept = true;
-              p.sp_cur[i] = ct;
-              const uint32_t rep = (uint32_t)x >> p.stride_shift;
-              atomicSub(&row[rep * p.n_species + s], 1u);
-              atomicAdd(&row[rep * p.n_species + ct], 1u);
-            }
-          }
-          if (accept) {
-            x = qx + rbase; y = qy; z = qz;
-            p.cur.x[i] = x; p.cur.y[i] = y; p.cur.z[i] = z;
+  constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
+  for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {   // block-uniform trip count
+    uint16_t s[kMoveUnroll];
+    int32_t x[kMoveUnroll], y[kMoveUnroll], z[kMoveUnroll];
+    uint32_t id[kMoveUnroll], key[kMoveUnroll];
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
+      s[a] = i < n ? p.cur.sp[i] : kDead;
+    }
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
+      if (s[a] != kDead) { x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; }
+    }
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      key[a] = 0xFFFFFFFFu;
+      if (s[a] == kDead) continue;
+      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
+      const DevSpecies& S = T->sp[s[a]];
+      const uint32_t cls = S.sigma_class;
+      if (cls) {
+        const uint4 r = philox4x32_10(id[a], 0u, t, kTagMove, p.key0, p.key1);
+        const int16_t* tb = g + (cls << p.table_bits);
+        const int32_t rbase = (int32_t)(((uint32_t)x[a] >> p.stride_shift) << p.stride_shift);
+        int32_t qx = x[a] - rbase + tb[r.x >> sh], qy = y[a] + tb[r.y >> sh], qz = z[a] + tb[r.z >> sh];
+        const DevComp& c = T->comp[S.compartment];
+        bool accept = true;
+        if (c.shape == 0) {
+          qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L);
+        } else if (!comp_valid(c, qx, qy, qz)) {
+          accept = false;
+          const uint16_t ct = S.cross_to;
+          if (ct != kDead && comp_valid(T->comp[T->sp[ct].compartment], qx, qy, qz) && fire(r.w, S.cross_thr)) {
+            accept = true;
+            p.cur.sp[i] = ct;
+            const uint32_t rep = (uint32_t)x[a] >> p.stride_shift;
+            atomicSub(&row[rep * p.n_species + s[a]], 1u);
+            atomicAdd(&row[rep * p.n_species + ct], 1u);
           }
         }
-        if (kHist) key = cell_key(x, y, z, p);
+        if (accept) {
+          x[a] = qx + rbase; y[a] = qy; z[a] = qz;
+          p.cur.x[i] = x[a]; p.cur.y[i] = y[a]; p.cur.z[i] = z[a];
+        }
       }
+      if (kHist) key[a] = cell_key(x[a], y[a], z[a], p);
     }
     if (kHist) {
-      const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
-      const int leader = __ffs(peers) - 1;
-      const uint32_t rank = __popc(peers & ((1u << lane) - 1u));
-      uint32_t first = 0;
-      if (live && (int)lane == leader) first = atomicAdd(&p.cell[key], (uint32_t)__popc(peers));
-      first = __shfl_sync(0xFFFFFFFFu, first, leader);
-      if (live) p.off[i] = first + rank;
+      uint32_t first[kMoveUnroll], rank[kMoveUnroll];
+      int leader[kMoveUnroll];
+#pragma unroll
+      for (int a = 0; a < kMoveUnroll; ++a) {
+        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key[a]);
+        leader[a] = __ffs(peers) - 1;
+        rank[a] = __popc(peers & ((1u << lane) - 1u));
+        first[a] = 0;
+        if (s[a] != kDead && (int)lane == leader[a]) first[a] = atomicAdd(&p.cell[key[a]], (uint32_t)__popc(peers));
+      }
+#pragma unroll
+      for (int a = 0; a < kMoveUnroll; ++a) {
+        const uint32_t f = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]);
+        if (s[a] != kDead) p.off[base + a * kMoveThreads + threadIdx.x] = f + rank[a];
+      }
     }
   }
 }
@@ -196,150 +218,402 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
 
 // ----------------------------------------------------------------------------- K3 scatter / reorder
 // Counting-sort scatter that reorders the whole structure of arrays into cell order (a5) and drops
-// DEAD slots, which is the compaction of the previous step's deaths (fused, a9).
-__global__ void __launch_bounds__(256) k_scatter(Params p) {
+// DEAD slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
+// kMoveUnroll agents in flight per thread.
+__global__ void __launch_bounds__(kMoveThreads) k_scatter(Params p) {
   const uint32_t n = p.scal->n_slots;
-  const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const uint16_t s = p.sp_cur[i];
-    if (s == kDead) continue;
-    const int32_t x = p.cur.x[i], y = p.cur.y[i], z = p.cur.z[i];
-    const uint32_t dst = p.cell[cell_key(x, y, z, p)] + p.off[i];
-    p.oth.x[dst] = x; p.oth.y[dst] = y; p.oth.z[dst] = z;
-    p.oth.id[dst] = p.cur.id[i];
-    p.sp_sorted[dst] = s;
+  constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
+  for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {
+    uint16_t s[kMoveUnroll];
+    int32_t x[kMoveUnroll], y[kMoveUnroll], z[kMoveUnroll];
+    uint32_t id[kMoveUnroll], off[kMoveUnroll];
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
+      s[a] = i < n ? p.cur.sp[i] : kDead;
+    }
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
+      if (s[a] != kDead) {
+        x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; off[a] = p.off[i];
+      }
+    }
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      if (s[a] != kDead) off[a] += p.cell[cell_key(x[a], y[a], z[a], p)];
+    }
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      if (s[a] == kDead) continue;
+      const uint32_t dst = off[a];
+      p.oth.x[dst] = x[a]; p.oth.y[dst] = y[a]; p.oth.z[dst] = z[a];
+      p.oth.id[dst] = id[a];
+      p.oth.sp[dst] = s[a];
+    }
   }
 }
 
-// ----------------------------------------------------------------------------- K4 neighbour + proposal
+// ----------------------------------------------------------------------------- counts aggregation
+// Per-step species counts (a10) are kept as deltas on a running row.  Events are aggregated in a
+// per-block shared-memory delta table and flushed once per block, so that thousands of bindings
+// per step do not serialise on a handful of global counters.
+constexpr int kMaxRowWidth = 64 * kMaxSpecies;   // SIM_MAX_REPLICAS x SIM_MAX_SPECIES
+__device__ __forceinline__ void delta_zero(int32_t* s_delta, uint32_t row_width) {
+  for (uint32_t k = threadIdx.x; k < row_width; k += blockDim.x) s_delta[k] = 0;
+  __syncthreads();
+}
+__device__ __forceinline__ void delta_flush(const int32_t* s_delta, uint32_t* __restrict__ row, uint32_t row_width) {
+  __syncthreads();
+  for (uint32_t k = threadIdx.x; k < row_width; k += blockDim.x) {
+    const int32_t d = s_delta[k];
+    if (d) atomicAdd(&row[k], (uint32_t)d);
+  }
+}
+
+// ----------------------------------------------------------------------------- K4 pair search + proposal
 // Phase 2a: each agent whose species can bind proposes its eligible partner with the smallest
 // (dist^2, id) among those that pass the symmetric pair draw (a6).  Only the cells its R-ball
 // overlaps are visited (exact: a cell it does not overlap cannot hold an in-range partner); with
 // x-fastest cell keys the cells of one (y,z) row are one contiguous slot range.
-__global__ void __launch_bounds__(128) k_neighbour(Params p) {
-  const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
+//
+// Work layout.  A block owns a tile of 256 consecutive sorted slots and stages their positions in
+// shared memory as int4 (x, y, z, species).
+//  A  own row, inside the tile: thread i tests only the slots AFTER its own (each unordered pair
+//     once); one 128-bit shared load, three adds, two max and one compare per candidate, no branch
+//     unless all three axes are within R.  The few slots of its range outside the tile are read
+//     from global memory, one direction only (the neighbouring tile does the other).
+//  B  the other (y,z) rows, which only agents near a cell face need, are pushed as 16-bit tasks
+//     (owner, row code) into a shared list and
+//  C  scanned one task per thread by the whole block, so the few lanes that need them do not stall
+//     their warps.
+//  D  geometric hits (dist^2 <= R^2: a fraction of a percent of the candidates) were only queued;
+//     now one thread per hit does the reaction lookup and the pair draw and merges the result into
+//     its owner(s) with a 64-bit shared atomicMin on (dist^2, partner id); the thread whose key won
+//     publishes the partner slot after a barrier.
+// A tile with more hits than the queue holds (dense test inputs) is redone by a plain per-thread
+// search.  Proposals are rare, so they are stored sparsely: prop[i] is written only when agent i
+// proposes and one ballot word per warp goes to the hasprop bitmap, which K4b scans.
+constexpr int kPairThreads = 256;
+constexpr int kTaskCap = 2048;          // 8 other rows x 256 agents
+constexpr int kHitCap = 768;
+constexpr unsigned long long kNoKey = ~0ull;
+
+// Reaction lookup, exact radius, symmetric pair draw for the geometric hit (i, j).  Returns the
+// proposal key of j as seen from i, (d2 << 32) | id_j, or kNoKey; *id_i_out = id of i.
+__device__ __forceinline__ unsigned long long pair_key(const Params& p, uint32_t i, uint32_t j, uint32_t d2,
+                                                       uint32_t si, uint32_t t, uint32_t* id_i_out) {
   const DevTables* __restrict__ T = p.tab;
+  const uint32_t e = T->rxmap[si * kMaxSpecies + p.oth.sp[j]];
+  if (e == 0xFFu) return kNoKey;
+  const DevRx& rx = T->rx[e];
+  if (d2 > rx.r2) return kNoKey;
+  const uint32_t id = p.oth.id[i], idj = p.oth.id[j];
+  const uint4 r = philox4x32_10(min(id, idj), max(id, idj), t, kTagPair, p.key0, p.key1);
+  if (!fire(r.x, rx.thr)) return kNoKey;
+  *id_i_out = id;
+  return ((unsigned long long)d2 << 32) | idj;
+}
+
+struct PairSmem {
+  int4 pos[kPairThreads];               // x, y, z, species
+  unsigned long long key[kPairThreads];
+  uint32_t row[kPairThreads], xr[kPairThreads], slot[kPairThreads];
+  uint32_t hit_j[kHitCap], hit_d[kHitCap];
+  uint16_t hit_o[kHitCap];              // owner thread | both-directions flag << 15
+  uint16_t task[kTaskCap];              // owner thread | row code (0..8) << 8
+  uint32_t ntask, nhit;
+};
+
+__device__ __forceinline__ void push_hit(PairSmem& S, uint32_t owner, uint32_t j, uint32_t d2, uint32_t both) {
+  const uint32_t h = atomicAdd(&S.nhit, 1u);
+  if (h < (uint32_t)kHitCap) { S.hit_j[h] = j; S.hit_d[h] = d2; S.hit_o[h] = (uint16_t)(owner | (both << 15)); }
+}
+
+// One-direction scan of global slots [j0, j1) for the agent `owner` of the tile at (x, y, z).
+__device__ __forceinline__ void scan_global(const Params& p, PairSmem& S, uint32_t j0, uint32_t j1, uint32_t owner,
+                                            int32_t x, int32_t y, int32_t z) {
   const int32_t R = p.max_r;
-  const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const uint16_t s = p.sp_sorted[i];
-    uint32_t best_j = kNoProp;
-    if (T->sp[s].binds) {
-      const int32_t x = p.oth.x[i], y = p.oth.y[i], z = p.oth.z[i];
-      const uint32_t id = p.oth.id[i];
-      const int32_t xlo = cell_coord(max(x - R, 0), p), xhi = min(cell_coord(x + R, p), p.nx - 1);
-      const int32_t ylo = cell_coord(max(y - R, 0), p), yhi = min(cell_coord(y + R, p), p.ny - 1);
-      const int32_t zlo = cell_coord(max(z - R, 0), p), zhi = min(cell_coord(z + R, p), p.nz - 1);
-      unsigned long long best = ~0ull;
-      const uint8_t* __restrict__ rxrow = T->rxmap + (uint32_t)s * kMaxSpecies;
-      for (int32_t cz = zlo; cz <= zhi; ++cz) {
-        for (int32_t cy = ylo; cy <= yhi; ++cy) {
-          const uint32_t rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
-          const uint32_t j0 = p.cell[rowc + xlo], j1 = p.cell[rowc + xhi + 1];
-          for (uint32_t j = j0; j < j1; ++j) {
-            const int32_t dx = p.oth.x[j] - x;
-            if (abs(dx) > R) continue;
-            const int32_t dy = p.oth.y[j] - y;
-            if (abs(dy) > R) continue;
-            const int32_t dz = p.oth.z[j] - z;
-            if (abs(dz) > R) continue;
-            const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-            if (d2 > p.max_r2 || j == i) continue;
-            const uint32_t e = rxrow[p.sp_sorted[j]];
-            if (e == 0xFFu) continue;
-            const DevRx& rx = T->rx[e];
-            if (d2 > rx.r2) continue;
-            const uint32_t idj = p.oth.id[j];
-            const uint4 r = philox4x32_10(min(id, idj), max(id, idj), t, kTagPair, p.key0, p.key1);
-            if (!fire(r.x, rx.thr)) continue;
-            const unsigned long long k = ((unsigned long long)d2 << 32) | idj;
-            if (k < best) { best = k; best_j = j; }
-          }
-        }
-      }
+  const uint32_t R2 = 2u * (uint32_t)R;
+  const int32_t ox = R - x, oy = R - y, oz = R - z;
+  const int32_t* __restrict__ X = p.oth.x;
+  const int32_t* __restrict__ Y = p.oth.y;
+  const int32_t* __restrict__ Z = p.oth.z;
+#pragma unroll 2
+  for (uint32_t j = j0; j < j1; ++j) {
+    const uint32_t ux = (uint32_t)(__ldg(X + j) + ox), uy = (uint32_t)(__ldg(Y + j) + oy), uz = (uint32_t)(__ldg(Z + j) + oz);
+    if (max(max(ux, uy), uz) <= R2) {
+      const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
+      const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
+      if (d2 <= p.max_r2) push_hit(S, owner, j, d2, 0u);
     }
-    p.prop[i] = best_j;
   }
 }
 
-// ----------------------------------------------------------------------------- K5 resolve + unimolecular
-// Phase 2b (mutual proposals bind, a7) and phase 3 (unimolecular channels, a8).  Species are read
-// from the sorted copy and written to sp_cur, so a partner's pre-binding species is never
-// overwritten while it is still needed.  Firing parents are appended to the birth list and flagged
-// in the id-indexed birth bitmap (4 bits per id) that K6 ranks.  Counts row t+1 receives deltas.
-__global__ void __launch_bounds__(256) k_resolve_uni(Params p) {
-  const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
-  const DevTables* __restrict__ T = p.tab;
-  uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
-  const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const uint16_t s0 = p.sp_sorted[i];
-    uint16_t s = s0;
-    const uint32_t pr = p.prop[i];
-    uint32_t id = 0;
-    bool have_id = false;
-    if (pr != kNoProp && p.prop[pr] == i) {
-      const uint16_t sj = p.sp_sorted[pr];
-      const DevRx& rx = T->rx[T->rxmap[(uint32_t)s * kMaxSpecies + sj]];
-      id = p.oth.id[i]; have_id = true;
-      const bool anchor = (s != sj) ? (s == rx.a) : (id < p.oth.id[pr]);
-      s = anchor ? rx.cplx : kDead;
-    }
-    uint32_t mask = 0;
-    const uint16_t pre = s;
-    if (s != kDead) {
-      const DevSpecies& S = T->sp[s];
-      const uint32_t nch = S.n_channels;
-      if (nch) {
-        if (!have_id) id = p.oth.id[i];
-        const uint4 r = philox4x32_10(id, 0u, t, kTagUni, p.key0, p.key1);
-        const uint32_t rr[4] = {r.x, r.y, r.z, r.w};
-        bool consumed = false;
-        uint16_t news = s;
-#pragma unroll
-        for (uint32_t k = 0; k < 4u; ++k) {
-          if (k >= nch) break;
-          const DevChannel ch = S.ch[k];
-          if (ch.kind == kChNone) continue;
-          bool fired;
-          if (ch.kind == kChDelayed) {
-            const uint32_t tf = *((volatile uint32_t*)&p.scal->t_first[ch.rule]);
-            fired = tf != kNever && t == tf + ch.thr;
-          } else {
-            fired = fire(rr[k], ch.thr);
-          }
-          if (!fired) continue;
-          switch (ch.kind) {
-            case kChBirth:
-              mask |= 1u << k;
-              if (ch.marks_first) atomicMin(&p.scal->t_first[ch.rule], t);
-              break;
-            case kChDelayed: mask |= 1u << k; break;
-            case kChRelease: if (!consumed) { consumed = true; news = ch.prod0; mask |= 1u << k; } break;
-            case kChConvert: if (!consumed) { consumed = true; news = ch.prod0; } break;
-            case kChDegrade: if (!consumed) { consumed = true; news = kDead; } break;
-          }
-        }
-        s = news;
-      }
-    }
-    p.sp_cur[i] = s;
-    if (s != s0 || mask) {
-      const uint32_t rep = (uint32_t)p.oth.x[i] >> p.stride_shift;
-      uint32_t* rr = row + rep * p.n_species;
-      if (s != s0) {
-        atomicSub(&rr[s0], 1u);
-        if (s != kDead) atomicAdd(&rr[s], 1u);
-      }
-      if (mask) {
-        const DevSpecies& P = T->sp[pre];
-        for (uint32_t k = 0; k < 4u; ++k) if (mask >> k & 1u) atomicAdd(&rr[P.ch[k].prod1], 1u);
-        atomicOr(&p.bits[id >> 3], mask << ((id & 7u) * 4u));
-        const uint32_t e = atomicAdd(&p.scal->birth_count, 1u);
-        p.birth_list[e] = make_uint2(i, mask | ((uint32_t)pre << 16));
-      }
+// Plain per-thread search of every overlapped row (the definition, as in DESIGN.md §1 phase 2):
+// used for tiles whose hit queue overflowed.
+__device__ __noinline__ void slow_agent(const Params* pp, uint32_t i, int32_t x, int32_t y, int32_t z, uint32_t si,
+                                        uint32_t rowc, uint32_t xlo, uint32_t nxr, uint32_t need, uint32_t t,
+                                        unsigned long long* best_out, uint32_t* slot_out) {
+  const Params& p = *pp;
+  unsigned long long best = kNoKey;
+  uint32_t best_j = kNoProp;
+  const long long R = p.max_r;
+  need |= 1u << 4;
+  while (need) {
+    const uint32_t c = __ffs(need) - 1u;
+    need &= need - 1u;
+    const uint32_t r2 = rowc + (uint32_t)(((int32_t)(c % 3u) - 1) * p.nx + ((int32_t)(c / 3u) - 1) * p.nx * p.ny);
+    const uint32_t j0 = p.cell[r2 + xlo], j1 = p.cell[r2 + xlo + nxr + 1];
+    for (uint32_t j = j0; j < j1; ++j) {
+      if (j == i) continue;
+      const long long dx = (long long)p.oth.x[j] - x, dy = (long long)p.oth.y[j] - y, dz = (long long)p.oth.z[j] - z;
+      if (dx > R || dx < -R || dy > R || dy < -R || dz > R || dz < -R) continue;
+      const unsigned long long d2 = (unsigned long long)(dx * dx + dy * dy + dz * dz);
+      if (d2 > p.max_r2) continue;
+      uint32_t id_i;
+      const unsigned long long k = pair_key(p, i, j, (uint32_t)d2, si, t, &id_i);
+      if (k < best) { best = k; best_j = j; }
     }
   }
+  *best_out = best; *slot_out = best_j;
+}
+
+__global__ void __launch_bounds__(kPairThreads) k_pairs(Params p) {
+  __shared__ PairSmem S;
+  const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, tid = threadIdx.x;
+  const int32_t R = p.max_r, cs = p.cell_size;
+  const uint32_t R2 = 2u * (uint32_t)R;
+  for (uint32_t base = blockIdx.x * kPairThreads; base < n; base += gridDim.x * kPairThreads) {   // block-uniform
+    if (tid == 0) { S.ntask = 0; S.nhit = 0; }
+    const uint32_t i = base + tid;
+    uint32_t s = kDead;
+    int32_t x = 0x7FFFFFFF, y = 0, z = 0;      // padding slots sit outside every search window
+    if (i < n) { s = p.oth.sp[i]; x = p.oth.x[i]; y = p.oth.y[i]; z = p.oth.z[i]; }
+    const bool active = s != kDead && ((p.binds_mask >> s) & 1ull);
+    uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0;
+    if (active) {
+      // R <= cell_size (validated), so the R-ball reaches at most one cell further on each side
+      const int32_t cx = cell_coord(x, p), cy = cell_coord(y, p), cz = cell_coord(z, p);
+      const int32_t lx = x - cx * cs, ly = y - cy * cs, lz = z - cz * cs;
+      const uint32_t xm = lx < R && cx > 0, xp = lx >= cs - R && cx < p.nx - 1;
+      const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
+      const uint32_t zm = lz < R && cz > 0, zp = lz >= cs - R && cz < p.nz - 1;
+      xlo = (uint32_t)cx - xm; nxr = xm + xp;
+      rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
+      // bit (dz+1)*3 + (dy+1) of `need`: the row at offset (dy, dz) must be searched (bit 4 = own row)
+      const uint32_t ymask = ym | (yp << 2);
+      need = (zm ? (ymask | 2u) : 0u) | (ymask << 3) | (zp ? (ymask | 2u) << 6 : 0u);
+    }
+    S.pos[tid] = make_int4(x, y, z, (int32_t)s);
+    S.row[tid] = rowc; S.xr[tid] = xlo | (nxr << 30);
+    S.key[tid] = kNoKey; S.slot[tid] = kNoProp;
+    __syncthreads();
+
+    // ---- A: own row
+    if (active) {
+      const uint32_t j0 = p.cell[rowc + xlo], j1 = p.cell[rowc + xlo + nxr + 1];
+      const int32_t ox = R - x, oy = R - y, oz = R - z;
+      const uint32_t kb = min(j1, base + kPairThreads) - base;     // j1 > i >= base
+#pragma unroll 4
+      for (uint32_t k = tid + 1u; k < kb; ++k) {
+        const int4 q = S.pos[k];
+        const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
+        if (max(max(ux, uy), uz) <= R2) {
+          const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
+          const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
+          if (d2 <= p.max_r2) push_hit(S, tid, base + k, d2, 1u);
+        }
+      }
+      if (j0 < base) scan_global(p, S, j0, base, tid, x, y, z);
+      if (j1 > base + kPairThreads) scan_global(p, S, base + kPairThreads, j1, tid, x, y, z);
+    }
+
+    // ---- B: reserve task slots (warp-inclusive scan of the task counts, one shared atomic per warp)
+    const uint32_t my_tasks = __popc(need);
+    uint32_t incl = my_tasks;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+      if (lane >= (uint32_t)d) incl += o;
+    }
+    const uint32_t wtotal = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    uint32_t wbase = 0;
+    if (lane == 31 && wtotal) wbase = atomicAdd(&S.ntask, wtotal);
+    wbase = __shfl_sync(0xFFFFFFFFu, wbase, 31);
+    {
+      uint32_t pos = wbase + incl - my_tasks, m = need;      // <= 2048 tasks per tile: always fits
+      while (m) {
+        const uint32_t c = __ffs(m) - 1u;
+        m &= m - 1u;
+        S.task[pos++] = (uint16_t)(tid | (c << 8));
+      }
+    }
+    __syncthreads();
+
+    // ---- C: the other rows, one task per thread
+    const uint32_t nt = S.ntask;
+    for (uint32_t k = tid; k < nt; k += kPairThreads) {
+      const uint32_t e = S.task[k], c = e >> 8, owner = e & 0xFFu;
+      const uint32_t xr = S.xr[owner], oxlo = xr & 0x3FFFFFFFu, onx = xr >> 30;
+      const uint32_t r2 = S.row[owner] + (uint32_t)(((int32_t)(c % 3u) - 1) * p.nx + ((int32_t)(c / 3u) - 1) * p.nx * p.ny);
+      const int4 q = S.pos[owner];
+      scan_global(p, S, p.cell[r2 + oxlo], p.cell[r2 + oxlo + onx + 1], owner, q.x, q.y, q.z);
+    }
+    __syncthreads();
+
+    // ---- D: qualify the queued hits and merge them into their owners
+    const uint32_t nh = S.nhit;
+    if (nh <= (uint32_t)kHitCap) {
+      for (uint32_t h0 = 0; h0 < nh; h0 += kPairThreads) {      // block-uniform; one round in the common case
+        const uint32_t h = h0 + tid;
+        unsigned long long k_own = kNoKey, k_oth = kNoKey;
+        uint32_t owner = 0, other = 0, j = 0;
+        if (h < nh) {
+          const uint32_t e = S.hit_o[h];
+          owner = e & 0xFFu; j = S.hit_j[h];
+          uint32_t id_i = 0;
+          k_own = pair_key(p, base + owner, j, S.hit_d[h], (uint32_t)S.pos[owner].w, t, &id_i);
+          if (k_own != kNoKey) {
+            atomicMin(&S.key[owner], k_own);
+            if (e >> 15) {                                   // both in the tile: the partner sees the same pair
+              other = j - base;
+              k_oth = (k_own & 0xFFFFFFFF00000000ull) | id_i;
+              atomicMin(&S.key[other], k_oth);
+            }
+          }
+        }
+        __syncthreads();
+        if (k_own != kNoKey && S.key[owner] == k_own) S.slot[owner] = j;            // keys are unique per owner
+        if (k_oth != kNoKey && S.key[other] == k_oth) S.slot[other] = base + owner;
+        __syncthreads();
+      }
+    } else if (active) {
+      unsigned long long kb; uint32_t sb;
+      slow_agent(&p, i, x, y, z, s, rowc, xlo, nxr, need, t, &kb, &sb);
+      S.key[tid] = kb; S.slot[tid] = sb;                     // own entries only; nothing else touches them here
+    }
+    const bool found = S.key[tid] != kNoKey;
+    const uint32_t word = __ballot_sync(0xFFFFFFFFu, found);
+    if (lane == 0 && base + warp * 32u < n) p.hasprop[(base >> 5) + warp] = word;
+    if (found) p.prop[i] = S.slot[tid];
+    __syncthreads();   // shared arrays are reused by the next tile
+  }
+}
+
+// ----------------------------------------------------------------------------- K4b handshake resolve
+// Phase 2b: a binding happens iff the proposal is mutual (a7).  One thread per word of the hasprop
+// bitmap; the lower slot of a mutual pair rewrites both species in place (anchor -> complex, the
+// other -> DEAD; S10).  No other thread reads or writes the species of a matched agent in this
+// kernel: a third agent that proposed to one of them only reads prop[].
+__global__ void __launch_bounds__(256) k_resolve(Params p) {
+  __shared__ int32_t s_delta[kMaxRowWidth];
+  delta_zero(s_delta, p.row_width);
+  const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
+  const uint32_t nw = (n + 31u) >> 5;
+  const DevTables* __restrict__ T = p.tab;
+  for (uint32_t w = blockIdx.x * blockDim.x + threadIdx.x; w < nw; w += gridDim.x * blockDim.x) {
+    uint32_t bits = p.hasprop[w];
+    while (bits) {
+      const uint32_t b = __ffs(bits) - 1u;
+      bits &= bits - 1u;
+      const uint32_t i = w * 32u + b, j = p.prop[i];
+      if (j <= i) continue;                                   // the lower slot handles the pair
+      if (!((p.hasprop[j >> 5] >> (j & 31u)) & 1u) || p.prop[j] != i) continue;
+      const uint16_t si = p.oth.sp[i], sj = p.oth.sp[j];
+      const DevRx& rx = T->rx[T->rxmap[(uint32_t)si * kMaxSpecies + sj]];
+      const bool anchor_i = (si != sj) ? (si == rx.a) : (p.oth.id[i] < p.oth.id[j]);
+      p.oth.sp[i] = anchor_i ? rx.cplx : kDead;
+      p.oth.sp[j] = anchor_i ? kDead : rx.cplx;
+      int32_t* d = s_delta + ((uint32_t)p.oth.x[i] >> p.stride_shift) * p.n_species;
+      atomicSub(&d[si], 1); atomicSub(&d[sj], 1); atomicAdd(&d[rx.cplx], 1);
+    }
+  }
+  delta_flush(s_delta, p.counts + (size_t)(t + 1) * p.row_width, p.row_width);
+}
+
+// ----------------------------------------------------------------------------- K5 unimolecular
+// Phase 3 (a8): per agent, per channel, Philox(seed, t, id) word < threshold.  Most agents belong to
+// a species without channels: a thread reads the species of 8 agents with one 128-bit load and
+// touches id / position only for those that have channels (chan_mask).  Species are rewritten in
+// place only where they change.  Firing parents are appended to the birth list and flagged in the
+// id-indexed birth bitmap (4 bits per id) that K6 ranks.  Counts deltas are block-aggregated.
+__device__ __forceinline__ void uni_one(const Params& p, const DevTables* __restrict__ T, uint32_t i, uint16_t s0,
+                                        uint32_t t, int32_t* s_delta) {
+  const DevSpecies& S = T->sp[s0];
+  const uint32_t nch = S.n_channels;
+  const uint32_t id = p.oth.id[i];
+  const uint4 r = philox4x32_10(id, 0u, t, kTagUni, p.key0, p.key1);
+  const uint32_t rr[4] = {r.x, r.y, r.z, r.w};
+  bool consumed = false;
+  uint16_t s = s0;
+  uint32_t mask = 0;
+#pragma unroll
+  for (uint32_t k = 0; k < 4u; ++k) {
+    if (k >= nch) break;
+    const DevChannel ch = S.ch[k];
+    if (ch.kind == kChNone) continue;
+    bool fired;
+    if (ch.kind == kChDelayed) {
+      const uint32_t tf = *((volatile uint32_t*)&p.scal->t_first[ch.rule]);
+      fired = tf != kNever && t == tf + ch.thr;
+    } else {
+      fired = fire(rr[k], ch.thr);
+    }
+    if (!fired) continue;
+    switch (ch.kind) {
+      case kChBirth:
+        mask |= 1u << k;
+        if (ch.marks_first) atomicMin(&p.scal->t_first[ch.rule], t);
+        break;
+      case kChDelayed: mask |= 1u << k; break;
+      case kChRelease: if (!consumed) { consumed = true; s = ch.prod0; mask |= 1u << k; } break;
+      case kChConvert: if (!consumed) { consumed = true; s = ch.prod0; } break;
+      case kChDegrade: if (!consumed) { consumed = true; s = kDead; } break;
+    }
+  }
+  if (s == s0 && !mask) return;
+  int32_t* d = s_delta + ((uint32_t)p.oth.x[i] >> p.stride_shift) * p.n_species;
+  if (s != s0) {
+    p.oth.sp[i] = s;
+    atomicSub(&d[s0], 1);
+    if (s != kDead) atomicAdd(&d[s], 1);
+  }
+  if (mask) {
+    for (uint32_t k = 0; k < 4u; ++k) if (mask >> k & 1u) atomicAdd(&d[S.ch[k].prod1], 1);
+    atomicOr(&p.bits[id >> 3], mask << ((id & 7u) * 4u));
+    const uint32_t e = atomicAdd(&p.scal->birth_count, 1u);
+    p.birth_list[e] = make_uint2(i, mask | ((uint32_t)s0 << 16));
+  }
+}
+
+__global__ void __launch_bounds__(256) k_uni(Params p) {
+  __shared__ int32_t s_delta[kMaxRowWidth];
+  delta_zero(s_delta, p.row_width);
+  const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
+  const DevTables* __restrict__ T = p.tab;
+  const uint32_t ng = (n + 7u) >> 3;
+  for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
+    const uint32_t i0 = g * 8u;
+    uint32_t w[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+    if (i0 + 8u <= n) {
+      const uint4 q = *reinterpret_cast<const uint4*>(p.oth.sp + i0);
+      w[0] = q.x; w[1] = q.y; w[2] = q.z; w[3] = q.w;
+    } else {
+      for (uint32_t k = 0; i0 + k < n; ++k) {
+        const uint32_t v = p.oth.sp[i0 + k];
+        w[k >> 1] = (k & 1u) ? ((w[k >> 1] & 0x0000FFFFu) | (v << 16)) : ((w[k >> 1] & 0xFFFF0000u) | v);
+      }
+    }
+#pragma unroll
+    for (uint32_t k = 0; k < 8u; ++k) {
+      const uint32_t s = (w[k >> 1] >> ((k & 1u) * 16u)) & 0xFFFFu;
+      if (s == kDead || !((p.chan_mask >> s) & 1ull)) continue;
+      uni_one(p, T, i0 + k, (uint16_t)s, t, s_delta);
+    }
+  }
+  delta_flush(s_delta, p.counts + (size_t)(t + 1) * p.row_width, p.row_width);
 }
 
 // ----------------------------------------------------------------------------- K6 birth ranking
@@ -426,7 +700,7 @@ __global__ void __launch_bounds__(128) k_births(Params p) {
       const uint32_t dst = n_sorted + rank;
       p.oth.x[dst] = qx + rbase; p.oth.y[dst] = qy; p.oth.z[dst] = qz;
       p.oth.id[dst] = next_id + rank;
-      p.sp_cur[dst] = sp_new;
+      p.oth.sp[dst] = sp_new;
       ++rank;
     }
   }
@@ -488,19 +762,21 @@ __global__ void k_seed(Params p, uint32_t species, uint32_t replica, uint32_t co
     }
     const uint32_t d = dst_base + n;
     p.cur.x[d] = x + rbase; p.cur.y[d] = y; p.cur.z[d] = z; p.cur.id[d] = id;
-    p.sp_cur[d] = (uint16_t)species;
+    p.cur.sp[d] = (uint16_t)species;
   }
 }
 
 // Full histogram of the current state into counts row `r` (after seeding / loading), and its copy
 // into row r+1 as the base of the next step's deltas.
-__global__ void k_count_row(Params p, uint32_t r, uint32_t n_slots) {
-  uint32_t* row = p.counts + (size_t)r * p.row_width;
+__global__ void __launch_bounds__(256) k_count_row(Params p, uint32_t r, uint32_t n_slots) {
+  __shared__ int32_t s_delta[kMaxRowWidth];
+  delta_zero(s_delta, p.row_width);
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += gridDim.x * blockDim.x) {
-    const uint16_t s = p.sp_cur[i];
+    const uint16_t s = p.cur.sp[i];
     if (s == kDead) continue;
-    atomicAdd(&row[((uint32_t)p.cur.x[i] >> p.stride_shift) * p.n_species + s], 1u);
+    atomicAdd(&s_delta[((uint32_t)p.cur.x[i] >> p.stride_shift) * p.n_species + s], 1);
   }
+  delta_flush(s_delta, p.counts + (size_t)r * p.row_width, p.row_width);
 }
 __global__ void k_copy_row(Params p, uint32_t r) {
   const uint32_t* src = p.counts + (size_t)r * p.row_width;
@@ -508,14 +784,19 @@ __global__ void k_copy_row(Params p, uint32_t r) {
   for (uint32_t k = threadIdx.x; k < p.row_width; k += blockDim.x) dst[k] = src[k];
 }
 
-// sim_read_agents: gather live agents into the scratch (oth / sp_sorted) arrays.
-__global__ void k_gather_live(Params p, uint32_t n_slots) {
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += gridDim.x * blockDim.x) {
-    const uint16_t s = p.sp_cur[i];
+// sim_read_agents: gather live agents into the scratch (oth) arrays (warp-aggregated append).
+__global__ void __launch_bounds__(256) k_gather_live(Params p, uint32_t n_slots) {
+  const uint32_t lane = threadIdx.x & 31u;
+  for (uint32_t base = blockIdx.x * blockDim.x; base < n_slots; base += gridDim.x * blockDim.x) {
+    const uint32_t i = base + threadIdx.x;
+    const uint16_t s = i < n_slots ? p.cur.sp[i] : kDead;
+    const uint32_t live = __ballot_sync(0xFFFFFFFFu, s != kDead);
+    uint32_t d = 0;
+    if (lane == 0 && live) d = atomicAdd(&p.scal->n_read, (uint32_t)__popc(live));
+    d = __shfl_sync(0xFFFFFFFFu, d, 0) + __popc(live & ((1u << lane) - 1u));
     if (s == kDead) continue;
-    const uint32_t d = atomicAdd(&p.scal->n_read, 1u);
     p.oth.x[d] = p.cur.x[i]; p.oth.y[d] = p.cur.y[i]; p.oth.z[d] = p.cur.z[i];
-    p.oth.id[d] = p.cur.id[i]; p.sp_sorted[d] = s;
+    p.oth.id[d] = p.cur.id[i]; p.oth.sp[d] = s;
   }
 }
 

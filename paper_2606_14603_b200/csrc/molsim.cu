@@ -18,16 +18,16 @@ namespace {
 constexpr int kScanBlocks = 592;          // 148 SMs x 4
 constexpr uint32_t kBirthBlocks = 296;    // 148 SMs x 2
 
-enum KernelId { KI_MOVE = 0, KI_CELL_ZERO, KI_CELL_REDUCE, KI_CELL_SCAN, KI_SCATTER, KI_NEIGHBOUR,
-                KI_RESOLVE, KI_BIRTH_REDUCE, KI_BIRTH_SCAN, KI_BIRTHS, KI_EPILOGUE, KI_OTHER };
+enum KernelId { KI_MOVE = 0, KI_CELL_ZERO, KI_CELL_REDUCE, KI_CELL_SCAN, KI_SCATTER, KI_PAIRS,
+                KI_RESOLVE, KI_UNI, KI_BIRTH_REDUCE, KI_BIRTH_SCAN, KI_BIRTHS, KI_EPILOGUE, KI_OTHER };
 const char* kKernelNames[SIM_N_KERNELS] = {
-    "k_move_hist", "memset_cells", "k_cell_reduce", "k_cell_scan", "k_scatter", "k_neighbour",
-    "k_resolve_uni", "k_birth_reduce", "k_birth_scan", "k_births", "k_epilogue", "other"};
+    "k_move_hist", "memset_cells", "k_cell_reduce", "k_cell_scan", "k_scatter", "k_pairs",
+    "k_resolve", "k_uni", "k_birth_reduce", "k_birth_scan", "k_births", "k_epilogue", "other"};
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t soa[2][4], sp_cur, sp_sorted, off, prop, cell, partial, bits, chunk_prefix, birth_list, counts,
+  size_t soa[2][5], off, prop, hasprop, cell, partial, bits, chunk_prefix, birth_list, counts,
       scal, tab, gauss, total;
   uint32_t n_cells, nx, ny, nz;
 };
@@ -36,14 +36,14 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   const uint64_t cs = c->cell_size;
   const uint64_t nx = (c->extent[0] + cs - 1) / cs, ny = (c->extent[1] + cs - 1) / cs, nz = (c->extent[2] + cs - 1) / cs;
   const uint64_t nc = nx * ny * nz;
-  if (nc == 0 || nc >= 0x7FFFFFF0ull) return false;
+  if (nc == 0 || nc >= 0x7FFFFFF0ull || nx >= (1ull << 30)) return false;
   L.nx = (uint32_t)nx; L.ny = (uint32_t)ny; L.nz = (uint32_t)nz; L.n_cells = (uint32_t)nc;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
   const size_t cap = c->capacity;
-  for (int b = 0; b < 2; ++b) for (int a = 0; a < 4; ++a) L.soa[b][a] = take(cap * 4);
-  L.sp_cur = take(cap * 2); L.sp_sorted = take(cap * 2);
+  for (int b = 0; b < 2; ++b) for (int a = 0; a < 5; ++a) L.soa[b][a] = take(cap * (a < 4 ? 4 : 2) + 64);
   L.off = take(cap * 4); L.prop = take(cap * 4);
+  L.hasprop = take((cap / 32 + 16) * 4);
   L.cell = take(((size_t)nc + 1 + 1024) * 4);
   L.partial = take(4096 * 4);
   const size_t n_chunks = ((size_t)c->id_capacity + 63) / 64 + 1;
@@ -67,7 +67,7 @@ int validate(const sim_config_t* c) {
   if (c->n_compartments == 0 || c->n_compartments > SIM_MAX_COMPARTMENTS || c->n_rules > SIM_MAX_RULES) return SIM_E_INVAL;
   if (c->table_bits < 1 || c->table_bits > 16 || c->n_sigma_classes < 1 || c->n_sigma_classes > 255) return SIM_E_INVAL;
   if (c->n_replicas < 1 || c->n_replicas > SIM_MAX_REPLICAS || c->stride_shift > 31) return SIM_E_INVAL;
-  if (c->cell_size == 0 || c->cell_size > 16384) return SIM_E_INVAL;
+  if (c->cell_size < 2 || c->cell_size > 16384) return SIM_E_INVAL;
   if (c->capacity == 0 || c->capacity > 0x7FFFFFFFu || c->counts_rows == 0 || c->id_capacity == 0) return SIM_E_INVAL;
   for (int a = 0; a < 3; ++a) if (c->extent[a] <= 0) return SIM_E_INVAL;
   if (c->n_replicas > 1 && ((uint64_t)c->n_replicas << c->stride_shift) > 0x80000000ull) return SIM_E_INVAL;
@@ -140,7 +140,7 @@ struct sim {
   uint64_t launches = 0;
   int gauss_in_smem = 0;
   size_t gauss_bytes = 0;
-  uint32_t grid_agents = 0;
+  uint32_t grid_move = 0, grid_scatter = 0, grid_pairs = 0, grid_uni = 0, grid_resolve = 0;
   uint32_t cell_seg = 0;
   bool profile = false;
   float prof_ms[SIM_N_KERNELS] = {};
@@ -207,20 +207,20 @@ int recount_row(sim* s, uint32_t r, uint32_t n_slots) {
 
 int enqueue_step(sim* s) {
   Params& p = s->prm;
-  const uint32_t ga = s->grid_agents;
   {
     ProfScope ps(s, KI_CELL_ZERO, false);
     CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->stream));
   }
   { ProfScope ps(s, KI_MOVE);
-    k_move_hist<true><<<ga, 256, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(p, s->gauss_in_smem); }
+    k_move_hist<true><<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(p, s->gauss_in_smem); }
   { ProfScope ps(s, KI_CELL_REDUCE);
     k_cell_reduce<<<kScanBlocks, kScanThreads, 0, s->stream>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_CELL_SCAN);
     k_cell_scan<<<kScanBlocks, kScanThreads, 0, s->stream>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
-  { ProfScope ps(s, KI_SCATTER); k_scatter<<<ga, 256, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_NEIGHBOUR); k_neighbour<<<ga * 2, 128, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_RESOLVE); k_resolve_uni<<<ga, 256, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_SCATTER); k_scatter<<<s->grid_scatter, kMoveThreads, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->stream>>>(p); }
+  { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->stream>>>(p); }
   { ProfScope ps(s, KI_BIRTH_REDUCE); k_birth_reduce<<<kBirthBlocks, kScanThreads, 0, s->stream>>>(p); }
   { ProfScope ps(s, KI_BIRTH_SCAN); k_birth_scan<<<kBirthBlocks, kScanThreads, 0, s->stream>>>(p); }
   { ProfScope ps(s, KI_BIRTHS); k_births<<<148, 128, 0, s->stream>>>(p); }
@@ -297,10 +297,10 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   std::memset(&p, 0, sizeof(p));
   char* w = s->ws;
   auto soa = [&](int b) { return Soa{(int32_t*)(w + L.soa[b][0]), (int32_t*)(w + L.soa[b][1]),
-                                     (int32_t*)(w + L.soa[b][2]), (uint32_t*)(w + L.soa[b][3])}; };
+                                     (int32_t*)(w + L.soa[b][2]), (uint32_t*)(w + L.soa[b][3]),
+                                     (uint16_t*)(w + L.soa[b][4])}; };
   p.cur = soa(0); p.oth = soa(1);
-  p.sp_cur = (uint16_t*)(w + L.sp_cur); p.sp_sorted = (uint16_t*)(w + L.sp_sorted);
-  p.off = (uint32_t*)(w + L.off); p.prop = (uint32_t*)(w + L.prop);
+  p.off = (uint32_t*)(w + L.off); p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
   p.cell = (uint32_t*)(w + L.cell); p.partial = (uint32_t*)(w + L.partial);
   p.bits = (uint32_t*)(w + L.bits); p.chunk_prefix = (uint32_t*)(w + L.chunk_prefix);
   p.birth_list = (uint2*)(w + L.birth_list); p.counts = (uint32_t*)(w + L.counts);
@@ -310,8 +310,16 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   p.n_species = cfg->n_species; p.n_replicas = cfg->n_replicas; p.stride_shift = cfg->stride_shift;
   p.table_bits = cfg->table_bits; p.n_classes = cfg->n_sigma_classes;
   p.cell_size = (int32_t)cfg->cell_size;
-  p.cell_shift = -1;
-  for (int b = 0; b < 31; ++b) if ((1u << b) == cfg->cell_size) p.cell_shift = b;
+  {
+    uint32_t l = 0;
+    while ((1ull << l) < cfg->cell_size) ++l;                       // l = ceil(log2 cell_size)
+    p.cell_mshift = l - 1u;                                          // cell_size >= 2 (validated), so l >= 1
+    p.cell_magic = (uint32_t)((1ull << (31u + l)) / cfg->cell_size + 1ull);
+  }
+  for (uint32_t i = 0; i < cfg->n_species; ++i) {
+    if (T.sp[i].binds) p.binds_mask |= 1ull << i;
+    if (T.sp[i].n_channels) p.chan_mask |= 1ull << i;
+  }
   p.nx = (int32_t)L.nx; p.ny = (int32_t)L.ny; p.nz = (int32_t)L.nz; p.n_cells = L.n_cells;
   p.max_r2 = max_r2;
   p.max_r = (int32_t)std::ceil(std::sqrt((double)max_r2));
@@ -320,16 +328,34 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
 
   s->gauss_bytes = ((size_t)cfg->n_sigma_classes << cfg->table_bits) * 2;
   s->gauss_in_smem = s->gauss_bytes <= 160 * 1024;
-  s->grid_agents = (uint32_t)std::min<uint64_t>(((uint64_t)cfg->capacity + 255) / 256, 148ull * 8);
+  // persistent grids: resident blocks per SM (occupancy API) x SM count, capped by the work there is
+  {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    auto sized = [&](int per_sm, uint64_t tile) {
+      const uint64_t need = ((uint64_t)cfg->capacity + tile - 1) / tile;
+      return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(need, (uint64_t)sms * (uint64_t)std::max(per_sm, 1)));
+    };
+    int occ = 0;
+    const size_t gsm = s->gauss_in_smem ? s->gauss_bytes : 0;
+    if (gsm > 48 * 1024) {
+      cudaFuncSetAttribute(k_move_hist<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(k_move_hist<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+    }
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hist<true>, kMoveThreads, gsm);
+    s->grid_move = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter, kMoveThreads, 0);
+    s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pairs, kPairThreads, 0);
+    s->grid_pairs = sized(occ, kPairThreads);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, 256, 0);
+    s->grid_uni = sized(occ, 256 * 8);
+    s->grid_resolve = sized(1, 256 * 32);
+    if (cudaGetLastError() != cudaSuccess) { delete s; return SIM_E_CUDA; }
+  }
   s->cell_seg = (uint32_t)align_up(((size_t)L.n_cells + kScanBlocks - 1) / kScanBlocks, 1024);
 
-  cudaError_t e;
-  if (s->gauss_in_smem && s->gauss_bytes > 48 * 1024) {
-    e = cudaFuncSetAttribute(k_move_hist<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->gauss_bytes);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(k_move_hist<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->gauss_bytes);
-    if (e != cudaSuccess) { delete s; return SIM_E_CUDA; }
-  }
   Scalars sc;
   std::memset(&sc, 0, sizeof(sc));
   for (int r = 0; r < kMaxRules; ++r) sc.t_first[r] = kNever;
@@ -466,7 +492,7 @@ int sim_read_agents(sim_t* s, uint32_t cap, int32_t* x, int32_t* y, int32_t* z, 
   }
   if (species) {
     std::vector<uint16_t> ts(n);
-    CK(cudaMemcpy(ts.data(), s->prm.sp_sorted, (size_t)n * 2, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(ts.data(), s->prm.oth.sp, (size_t)n * 2, cudaMemcpyDeviceToHost));
     for (uint32_t i = 0; i < n; ++i) species[i] = ts[order[i]];
   }
   if (id) for (uint32_t i = 0; i < n; ++i) id[i] = hid[order[i]];
@@ -486,7 +512,7 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
   CK(cudaMemcpyAsync(s->prm.cur.y, y, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
   CK(cudaMemcpyAsync(s->prm.cur.z, z, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
   CK(cudaMemcpyAsync(s->prm.cur.id, id, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->prm.sp_cur, species, (size_t)n * 2, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->prm.cur.sp, species, (size_t)n * 2, cudaMemcpyHostToDevice, s->stream));
   sc.n_slots = n; sc.next_id = next_id; sc.t = step; sc.err = 0;
   sc.birth_count = sc.total_births = sc.ticket = 0;
   CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
@@ -500,7 +526,7 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
 int sim_debug_move_only(sim_t* s) {
   if (!s) return SIM_E_INVAL;
   { ProfScope ps(s, KI_MOVE);
-    k_move_hist<false><<<s->grid_agents, 256, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(s->prm, s->gauss_in_smem); }
+    k_move_hist<false><<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(s->prm, s->gauss_in_smem); }
   CK(cudaGetLastError());
   // crossing deltas went to row t+1: fold them back so that row t describes the moved state
   Scalars sc;
