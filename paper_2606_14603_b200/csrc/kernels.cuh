@@ -379,7 +379,7 @@ __device__ __noinline__ void slow_agent(const Params* pp, uint32_t i, int32_t x,
   *best_out = best; *slot_out = best_j;
 }
 
-__global__ void __launch_bounds__(kPairThreads) k_pairs(Params p) {
+__global__ void __launch_bounds__(kPairThreads, 5) k_pairs(Params p) {
   __shared__ PairSmem S;
   const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, tid = threadIdx.x;
@@ -452,14 +452,15 @@ __global__ void __launch_bounds__(kPairThreads) k_pairs(Params p) {
     }
     __syncthreads();
 
-    // ---- C: the other rows, one task per thread
-    const uint32_t nt = S.ntask;
-    for (uint32_t k = tid; k < nt; k += kPairThreads) {
-      const uint32_t e = S.task[k], c = e >> 8, owner = e & 0xFFu;
+    // ---- C: the other rows, two threads per task (each scans half of the range)
+    const uint32_t nt2 = S.ntask * 2u;
+    for (uint32_t k = tid; k < nt2; k += kPairThreads) {
+      const uint32_t e = S.task[k >> 1], c = e >> 8, owner = e & 0xFFu;
       const uint32_t xr = S.xr[owner], oxlo = xr & 0x3FFFFFFFu, onx = xr >> 30;
       const uint32_t r2 = S.row[owner] + (uint32_t)(((int32_t)(c % 3u) - 1) * p.nx + ((int32_t)(c / 3u) - 1) * p.nx * p.ny);
       const int4 q = S.pos[owner];
-      scan_global(p, S, p.cell[r2 + oxlo], p.cell[r2 + oxlo + onx + 1], owner, q.x, q.y, q.z);
+      const uint32_t j0 = p.cell[r2 + oxlo], j1 = p.cell[r2 + oxlo + onx + 1], mid = (j0 + j1 + 1u) >> 1;
+      scan_global(p, S, (k & 1u) ? mid : j0, (k & 1u) ? j1 : mid, owner, q.x, q.y, q.z);
     }
     __syncthreads();
 
