@@ -278,25 +278,23 @@ __device__ __forceinline__ void delta_flush(const int32_t* s_delta, uint32_t* __
 // x-fastest cell keys the cells of one (y,z) row are one contiguous slot range.
 //
 // Work layout.  A block owns a tile of 256 consecutive sorted slots and stages their positions in
-// shared memory as int4 (x, y, z, species).
-//  A  own row, inside the tile: thread i tests only the slots AFTER its own (each unordered pair
-//     once); one 128-bit shared load, three adds, two max and one compare per candidate, no branch
-//     unless all three axes are within R.  The few slots of its range outside the tile are read
-//     from global memory, one direction only (the neighbouring tile does the other).
+// shared memory as int4 (x, y, z, species); after that single barrier its warps work on their own:
+//  A  own row, inside the tile: one 128-bit shared load, three adds, two max and one compare per
+//     candidate, no branch unless all three axes are within R.  Slots of its own warp are tested
+//     one way only (each unordered pair once, by the lower slot); the few slots of its range
+//     outside the tile are read from global memory.
 //  B  the other (y,z) rows, which only agents near a cell face need, are pushed as 16-bit tasks
-//     (owner, row code) into a shared list and
-//  C  scanned one task per thread by the whole block, so the few lanes that need them do not stall
-//     their warps.
+//     (owner, row code) into the warp's shared list and
+//  C  scanned by the whole warp, 1, 2 or 4 lanes per task, so the few lanes that need them do not
+//     stall the others.
 //  D  geometric hits (dist^2 <= R^2: a fraction of a percent of the candidates) were only queued;
-//     now one thread per hit does the reaction lookup and the pair draw and merges the result into
-//     its owner(s) with a 64-bit shared atomicMin on (dist^2, partner id); the thread whose key won
-//     publishes the partner slot after a barrier.
-// A tile with more hits than the queue holds (dense test inputs) is redone by a plain per-thread
-// search.  Proposals are rare, so they are stored sparsely: prop[i] is written only when agent i
-// proposes and one ballot word per warp goes to the hasprop bitmap, which K4b scans.
+//     now one lane per hit does the reaction lookup and the pair draw and merges the result into
+//     its owner(s) with a 64-bit shared atomicMin on (dist^2, partner id); the lane whose key won
+//     publishes the partner slot.
+// A warp with more hits than its queue holds (dense test inputs) redoes its agents by a plain
+// per-thread search.  Proposals are rare, so they are stored sparsely: prop[i] is written only when
+// agent i proposes and one ballot word per warp goes to the hasprop bitmap, which K4b scans.
 constexpr int kPairThreads = 256;
-constexpr int kTaskCap = 2048;          // 8 other rows x 256 agents
-constexpr int kHitCap = 768;
 constexpr unsigned long long kNoKey = ~0ull;
 
 // Reaction lookup, exact radius, symmetric pair draw for the geometric hit (i, j).  Returns the
@@ -315,23 +313,47 @@ __device__ __forceinline__ unsigned long long pair_key(const Params& p, uint32_t
   return ((unsigned long long)d2 << 32) | idj;
 }
 
+constexpr int kWarpTaskCap = 256;       // 8 other rows x 32 agents: always fits
+constexpr int kWarpHitCap = 64;
+struct PairWarpSmem {                   // private to one warp
+  uint32_t hit_j[kWarpHitCap], hit_d[kWarpHitCap];
+  uint16_t hit_o[kWarpHitCap];          // owner thread | both-directions flag << 15
+  uint16_t task[kWarpTaskCap];          // owner thread | row code (0..8) << 8
+  uint32_t nhit;
+};
 struct PairSmem {
   int4 pos[kPairThreads];               // x, y, z, species
   unsigned long long key[kPairThreads];
   uint32_t row[kPairThreads], xr[kPairThreads], slot[kPairThreads];
-  uint32_t hit_j[kHitCap], hit_d[kHitCap];
-  uint16_t hit_o[kHitCap];              // owner thread | both-directions flag << 15
-  uint16_t task[kTaskCap];              // owner thread | row code (0..8) << 8
-  uint32_t ntask, nhit;
+  PairWarpSmem w[kPairThreads / 32];
 };
 
-__device__ __forceinline__ void push_hit(PairSmem& S, uint32_t owner, uint32_t j, uint32_t d2, uint32_t both) {
-  const uint32_t h = atomicAdd(&S.nhit, 1u);
-  if (h < (uint32_t)kHitCap) { S.hit_j[h] = j; S.hit_d[h] = d2; S.hit_o[h] = (uint16_t)(owner | (both << 15)); }
+__device__ __forceinline__ void push_hit(PairWarpSmem& W, uint32_t owner, uint32_t j, uint32_t d2, uint32_t both) {
+  const uint32_t h = atomicAdd(&W.nhit, 1u);
+  if (h < (uint32_t)kWarpHitCap) { W.hit_j[h] = j; W.hit_d[h] = d2; W.hit_o[h] = (uint16_t)(owner | (both << 15)); }
+}
+
+// Scan of tile slots [ka, kb) (shared memory) for the agent `owner` at (x, y, z).
+// A hit on a later slot of the owner's own warp stands for both directions of the pair.
+__device__ __forceinline__ void scan_tile(const Params& p, const PairSmem& S, PairWarpSmem& W, uint32_t ka, uint32_t kb,
+                                          uint32_t base, uint32_t owner, int32_t x, int32_t y, int32_t z) {
+  const int32_t R = p.max_r;
+  const uint32_t R2 = 2u * (uint32_t)R;
+  const int32_t ox = R - x, oy = R - y, oz = R - z;
+#pragma unroll 4
+  for (uint32_t k = ka; k < kb; ++k) {
+    const int4 q = S.pos[k];
+    const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
+    if (max(max(ux, uy), uz) <= R2) {
+      const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
+      const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
+      if (d2 <= p.max_r2) push_hit(W, owner, base + k, d2, (k > owner && k < (owner | 31u) + 1u) ? 1u : 0u);
+    }
+  }
 }
 
 // One-direction scan of global slots [j0, j1) for the agent `owner` of the tile at (x, y, z).
-__device__ __forceinline__ void scan_global(const Params& p, PairSmem& S, uint32_t j0, uint32_t j1, uint32_t owner,
+__device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, uint32_t j0, uint32_t j1, uint32_t owner,
                                             int32_t x, int32_t y, int32_t z) {
   const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
@@ -345,7 +367,7 @@ __device__ __forceinline__ void scan_global(const Params& p, PairSmem& S, uint32
     if (max(max(ux, uy), uz) <= R2) {
       const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (d2 <= p.max_r2) push_hit(S, owner, j, d2, 0u);
+      if (d2 <= p.max_r2) push_hit(W, owner, j, d2, 0u);
     }
   }
 }
@@ -379,128 +401,119 @@ __device__ __noinline__ void slow_agent(const Params* pp, uint32_t i, int32_t x,
   *best_out = best; *slot_out = best_j;
 }
 
-__global__ void __launch_bounds__(kPairThreads, 5) k_pairs(Params p) {
+
+__global__ void __launch_bounds__(kPairThreads, 6) k_pairs(const __grid_constant__ Params p) {
   __shared__ PairSmem S;
   const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
+  const uint32_t base = blockIdx.x * kPairThreads;
+  if (base >= n) return;
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, tid = threadIdx.x;
+  PairWarpSmem& W = S.w[warp];
   const int32_t R = p.max_r, cs = p.cell_size;
-  const uint32_t R2 = 2u * (uint32_t)R;
-  for (uint32_t base = blockIdx.x * kPairThreads; base < n; base += gridDim.x * kPairThreads) {   // block-uniform
-    if (tid == 0) { S.ntask = 0; S.nhit = 0; }
-    const uint32_t i = base + tid;
-    uint32_t s = kDead;
-    int32_t x = 0x7FFFFFFF, y = 0, z = 0;      // padding slots sit outside every search window
-    if (i < n) { s = p.oth.sp[i]; x = p.oth.x[i]; y = p.oth.y[i]; z = p.oth.z[i]; }
-    const bool active = s != kDead && ((p.binds_mask >> s) & 1ull);
-    uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0;
-    if (active) {
-      // R <= cell_size (validated), so the R-ball reaches at most one cell further on each side
-      const int32_t cx = cell_coord(x, p), cy = cell_coord(y, p), cz = cell_coord(z, p);
-      const int32_t lx = x - cx * cs, ly = y - cy * cs, lz = z - cz * cs;
-      const uint32_t xm = lx < R && cx > 0, xp = lx >= cs - R && cx < p.nx - 1;
-      const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
-      const uint32_t zm = lz < R && cz > 0, zp = lz >= cs - R && cz < p.nz - 1;
-      xlo = (uint32_t)cx - xm; nxr = xm + xp;
-      rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
-      // bit (dz+1)*3 + (dy+1) of `need`: the row at offset (dy, dz) must be searched (bit 4 = own row)
-      const uint32_t ymask = ym | (yp << 2);
-      need = (zm ? (ymask | 2u) : 0u) | (ymask << 3) | (zp ? (ymask | 2u) << 6 : 0u);
-    }
-    S.pos[tid] = make_int4(x, y, z, (int32_t)s);
-    S.row[tid] = rowc; S.xr[tid] = xlo | (nxr << 30);
-    S.key[tid] = kNoKey; S.slot[tid] = kNoProp;
-    __syncthreads();
+  if (lane == 0) W.nhit = 0;
+  const uint32_t i = base + tid;
+  uint32_t s = kDead;
+  int32_t x = 0, y = 0, z = 0;
+  if (i < n) { s = p.oth.sp[i]; x = p.oth.x[i]; y = p.oth.y[i]; z = p.oth.z[i]; }
+  const bool active = s != kDead && ((p.binds_mask >> s) & 1ull);
+  uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0;
+  if (active) {
+    // R <= cell_size (validated), so the R-ball reaches at most one cell further on each side
+    const int32_t cx = cell_coord(x, p), cy = cell_coord(y, p), cz = cell_coord(z, p);
+    const int32_t lx = x - cx * cs, ly = y - cy * cs, lz = z - cz * cs;
+    const uint32_t xm = lx < R && cx > 0, xp = lx >= cs - R && cx < p.nx - 1;
+    const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
+    const uint32_t zm = lz < R && cz > 0, zp = lz >= cs - R && cz < p.nz - 1;
+    xlo = (uint32_t)cx - xm; nxr = xm + xp;
+    rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
+    // bit (dz+1)*3 + (dy+1) of `need`: the row at offset (dy, dz) must be searched (bit 4 = own row)
+    const uint32_t ymask = ym | (yp << 2);
+    need = (zm ? (ymask | 2u) : 0u) | (ymask << 3) | (zp ? (ymask | 2u) << 6 : 0u);
+  }
+  S.pos[tid] = make_int4(x, y, z, (int32_t)s);
+  S.row[tid] = rowc; S.xr[tid] = xlo | (nxr << 30);
+  S.key[tid] = kNoKey; S.slot[tid] = kNoProp;
+  __syncthreads();          // the only block-wide barrier: the tile is read-only from here on
 
-    // ---- A: own row
-    if (active) {
-      const uint32_t j0 = p.cell[rowc + xlo], j1 = p.cell[rowc + xlo + nxr + 1];
-      const int32_t ox = R - x, oy = R - y, oz = R - z;
-      const uint32_t kb = min(j1, base + kPairThreads) - base;     // j1 > i >= base
-#pragma unroll 4
-      for (uint32_t k = tid + 1u; k < kb; ++k) {
-        const int4 q = S.pos[k];
-        const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
-        if (max(max(ux, uy), uz) <= R2) {
-          const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
-          const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-          if (d2 <= p.max_r2) push_hit(S, tid, base + k, d2, 1u);
-        }
-      }
-      if (j0 < base) scan_global(p, S, j0, base, tid, x, y, z);
-      if (j1 > base + kPairThreads) scan_global(p, S, base + kPairThreads, j1, tid, x, y, z);
-    }
+  // ---- A: own row
+  if (active) {
+    const uint32_t j0 = p.cell[rowc + xlo], j1 = p.cell[rowc + xlo + nxr + 1];   // j0 <= i < j1
+    const uint32_t ka = max(j0, base) - base, kb = min(j1, base + kPairThreads) - base, wlo = tid & ~31u;
+    if (ka < wlo) scan_tile(p, S, W, ka, wlo, base, tid, x, y, z);
+    scan_tile(p, S, W, tid + 1u, kb, base, tid, x, y, z);
+    if (j0 < base) scan_global(p, W, j0, base, tid, x, y, z);
+    if (j1 > base + kPairThreads) scan_global(p, W, base + kPairThreads, j1, tid, x, y, z);
+  }
 
-    // ---- B: reserve task slots (warp-inclusive scan of the task counts, one shared atomic per warp)
-    const uint32_t my_tasks = __popc(need);
-    uint32_t incl = my_tasks;
+  // ---- B: the warp's task list (exclusive scan of the task counts)
+  const uint32_t my_tasks = __popc(need);
+  uint32_t incl = my_tasks;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-      if (lane >= (uint32_t)d) incl += o;
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (lane >= (uint32_t)d) incl += o;
+  }
+  const uint32_t nt = __shfl_sync(0xFFFFFFFFu, incl, 31);
+  {
+    uint32_t pos = incl - my_tasks, m = need;
+    while (m) {
+      const uint32_t c = __ffs(m) - 1u;
+      m &= m - 1u;
+      W.task[pos++] = (uint16_t)(tid | (c << 8));
     }
-    const uint32_t wtotal = __shfl_sync(0xFFFFFFFFu, incl, 31);
-    uint32_t wbase = 0;
-    if (lane == 31 && wtotal) wbase = atomicAdd(&S.ntask, wtotal);
-    wbase = __shfl_sync(0xFFFFFFFFu, wbase, 31);
-    {
-      uint32_t pos = wbase + incl - my_tasks, m = need;      // <= 2048 tasks per tile: always fits
-      while (m) {
-        const uint32_t c = __ffs(m) - 1u;
-        m &= m - 1u;
-        S.task[pos++] = (uint16_t)(tid | (c << 8));
-      }
-    }
-    __syncthreads();
+  }
+  __syncwarp();
 
-    // ---- C: the other rows, two threads per task (each scans half of the range)
-    const uint32_t nt2 = S.ntask * 2u;
-    for (uint32_t k = tid; k < nt2; k += kPairThreads) {
-      const uint32_t e = S.task[k >> 1], c = e >> 8, owner = e & 0xFFu;
+  // ---- C: the other rows: 4, 2 or 1 lanes per task
+  {
+    const uint32_t lg = nt <= 8u ? 2u : (nt <= 16u ? 1u : 0u), items = nt << lg;
+    for (uint32_t k = lane; k < items; k += 32u) {
+      const uint32_t e = W.task[k >> lg], c = e >> 8, owner = e & 0xFFu, part = k & ((1u << lg) - 1u);
       const uint32_t xr = S.xr[owner], oxlo = xr & 0x3FFFFFFFu, onx = xr >> 30;
       const uint32_t r2 = S.row[owner] + (uint32_t)(((int32_t)(c % 3u) - 1) * p.nx + ((int32_t)(c / 3u) - 1) * p.nx * p.ny);
       const int4 q = S.pos[owner];
-      const uint32_t j0 = p.cell[r2 + oxlo], j1 = p.cell[r2 + oxlo + onx + 1], mid = (j0 + j1 + 1u) >> 1;
-      scan_global(p, S, (k & 1u) ? mid : j0, (k & 1u) ? j1 : mid, owner, q.x, q.y, q.z);
+      const uint32_t j0 = p.cell[r2 + oxlo], len = p.cell[r2 + oxlo + onx + 1] - j0;
+      scan_global(p, W, j0 + ((len * part) >> lg), j0 + ((len * (part + 1u)) >> lg), owner, q.x, q.y, q.z);
     }
-    __syncthreads();
+  }
+  __syncwarp();
 
-    // ---- D: qualify the queued hits and merge them into their owners
-    const uint32_t nh = S.nhit;
-    if (nh <= (uint32_t)kHitCap) {
-      for (uint32_t h0 = 0; h0 < nh; h0 += kPairThreads) {      // block-uniform; one round in the common case
-        const uint32_t h = h0 + tid;
-        unsigned long long k_own = kNoKey, k_oth = kNoKey;
-        uint32_t owner = 0, other = 0, j = 0;
-        if (h < nh) {
-          const uint32_t e = S.hit_o[h];
-          owner = e & 0xFFu; j = S.hit_j[h];
-          uint32_t id_i = 0;
-          k_own = pair_key(p, base + owner, j, S.hit_d[h], (uint32_t)S.pos[owner].w, t, &id_i);
-          if (k_own != kNoKey) {
-            atomicMin(&S.key[owner], k_own);
-            if (e >> 15) {                                   // both in the tile: the partner sees the same pair
-              other = j - base;
-              k_oth = (k_own & 0xFFFFFFFF00000000ull) | id_i;
-              atomicMin(&S.key[other], k_oth);
-            }
+  // ---- D: qualify the queued hits and merge them into their owners (all within this warp)
+  const uint32_t nh = W.nhit;
+  if (nh <= (uint32_t)kWarpHitCap) {
+    for (uint32_t h0 = 0; h0 < nh; h0 += 32u) {      // warp-uniform; one round in the common case
+      const uint32_t h = h0 + lane;
+      unsigned long long k_own = kNoKey, k_oth = kNoKey;
+      uint32_t owner = 0, other = 0, j = 0;
+      if (h < nh) {
+        const uint32_t e = W.hit_o[h];
+        owner = e & 0xFFu; j = W.hit_j[h];
+        uint32_t id_i = 0;
+        k_own = pair_key(p, base + owner, j, W.hit_d[h], (uint32_t)S.pos[owner].w, t, &id_i);
+        if (k_own != kNoKey) {
+          atomicMin(&S.key[owner], k_own);
+          if (e >> 15) {                                   // the partner sees the same pair
+            other = j - base;
+            k_oth = (k_own & 0xFFFFFFFF00000000ull) | id_i;
+            atomicMin(&S.key[other], k_oth);
           }
         }
-        __syncthreads();
-        if (k_own != kNoKey && S.key[owner] == k_own) S.slot[owner] = j;            // keys are unique per owner
-        if (k_oth != kNoKey && S.key[other] == k_oth) S.slot[other] = base + owner;
-        __syncthreads();
       }
-    } else if (active) {
-      unsigned long long kb; uint32_t sb;
-      slow_agent(&p, i, x, y, z, s, rowc, xlo, nxr, need, t, &kb, &sb);
-      S.key[tid] = kb; S.slot[tid] = sb;                     // own entries only; nothing else touches them here
+      __syncwarp();
+      if (k_own != kNoKey && S.key[owner] == k_own) S.slot[owner] = j;            // keys are unique per owner
+      if (k_oth != kNoKey && S.key[other] == k_oth) S.slot[other] = base + owner;
+      __syncwarp();
     }
-    const bool found = S.key[tid] != kNoKey;
-    const uint32_t word = __ballot_sync(0xFFFFFFFFu, found);
-    if (lane == 0 && base + warp * 32u < n) p.hasprop[(base >> 5) + warp] = word;
-    if (found) p.prop[i] = S.slot[tid];
-    __syncthreads();   // shared arrays are reused by the next tile
+  } else if (active) {
+    unsigned long long kb; uint32_t sb;
+    slow_agent(&p, i, x, y, z, s, rowc, xlo, nxr, need, t, &kb, &sb);
+    S.key[tid] = kb; S.slot[tid] = sb;
   }
+  __syncwarp();
+  const bool found = S.key[tid] != kNoKey;
+  const uint32_t word = __ballot_sync(0xFFFFFFFFu, found);
+  if (lane == 0 && base + warp * 32u < n) p.hasprop[(base >> 5) + warp] = word;
+  if (found) p.prop[i] = S.slot[tid];
 }
 
 // ----------------------------------------------------------------------------- K4b handshake resolve

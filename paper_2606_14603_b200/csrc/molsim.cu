@@ -347,8 +347,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     s->grid_move = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter, kMoveThreads, 0);
     s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pairs, kPairThreads, 0);
-    s->grid_pairs = sized(occ, kPairThreads);
+    s->grid_pairs = (uint32_t)(((uint64_t)cfg->capacity + kPairThreads - 1) / kPairThreads);   // one tile per block
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, 256, 0);
     s->grid_uni = sized(occ, 256 * 8);
     s->grid_resolve = sized(1, 256 * 32);
