@@ -273,68 +273,72 @@ __device__ __forceinline__ void delta_flush(const int32_t* s_delta, uint32_t* __
 
 // ----------------------------------------------------------------------------- K4 pair search + proposal
 // Phase 2a: each agent whose species can bind proposes its eligible partner with the smallest
-// (dist^2, id) among those that pass the symmetric pair draw (a6).  Only the cells its R-ball
-// overlaps are visited (exact: a cell it does not overlap cannot hold an in-range partner); with
-// x-fastest cell keys the cells of one (y,z) row are one contiguous slot range.
+// (dist^2, id) among those that pass the symmetric pair draw (a6).  The predicate and the draw are
+// symmetric in the pair, so every unordered pair is examined ONCE, by its lower sorted slot i < j,
+// and a qualifying pair is merged into both ends: best[i] <- min(., (d2, id_j)), best[j] <- min(.,
+// (d2, id_i)) with 64-bit global atomicMin.  Only cells the R-ball overlaps are visited (exact: a
+// cell it does not overlap cannot hold an in-range partner), and of those only the "forward" ones:
+// the rest of the agent's own cell, the +x cell, and the overlapped cells of the rows (y+1, z) and
+// (y-1..y+1, z+1).  With x-fastest cell keys the cells of one (y,z) row are one contiguous slot range.
 //
 // Work layout.  A block owns a tile of 256 consecutive sorted slots and stages their positions in
 // shared memory as int4 (x, y, z, species); after that single barrier its warps work on their own:
-//  A  own row, inside the tile: one 128-bit shared load, three adds, two max and one compare per
-//     candidate, no branch unless all three axes are within R.  Slots of its own warp are tested
-//     one way only (each unordered pair once, by the lower slot); the few slots of its range
-//     outside the tile are read from global memory.
-//  B  the other (y,z) rows, which only agents near a cell face need, are pushed as 16-bit tasks
-//     (owner, row code) into the warp's shared list and
+//  A  own row: slots (i, j1).  Inside the tile: one 128-bit shared load, three adds, two max and one
+//     compare per candidate, no branch unless all three axes are within R; the few slots past the
+//     tile end are read from global memory.
+//  B  the forward (y,z) rows, which only agents near a +y / +z (or, for the z+1 rows, -y) cell face
+//     need, are pushed as 16-bit tasks (owner, row code) into the warp's shared list and
 //  C  scanned by the whole warp, 1, 2 or 4 lanes per task, so the few lanes that need them do not
 //     stall the others.
 //  D  geometric hits (dist^2 <= R^2: a fraction of a percent of the candidates) were only queued;
-//     now one lane per hit does the reaction lookup and the pair draw and merges the result into
-//     its owner(s) with a 64-bit shared atomicMin on (dist^2, partner id); the lane whose key won
-//     publishes the partner slot.
+//     now one lane per hit does the reaction lookup and the pair draw and, if the pair qualifies,
+//     the two atomicMin.  best[] is touched only there (rare), so it costs no bandwidth; hasprop
+//     gets one bit per touched agent and bslot[] the slot of the partner that lowered the key.
+//     Two lanes lowering the same key may store their slots in either order, so K4b checks
+//     id[bslot[i]] against the key and searches the neighbourhood again in that (vanishingly rare) case.
 // A warp with more hits than its queue holds (dense test inputs) redoes its agents by a plain
-// per-thread search.  Proposals are rare, so they are stored sparsely: prop[i] is written only when
-// agent i proposes and one ballot word per warp goes to the hasprop bitmap, which K4b scans.
+// per-thread search.
 constexpr int kPairThreads = 256;
 constexpr unsigned long long kNoKey = ~0ull;
 
-// Reaction lookup, exact radius, symmetric pair draw for the geometric hit (i, j).  Returns the
-// proposal key of j as seen from i, (d2 << 32) | id_j, or kNoKey; *id_i_out = id of i.
-__device__ __forceinline__ unsigned long long pair_key(const Params& p, uint32_t i, uint32_t j, uint32_t d2,
-                                                       uint32_t si, uint32_t t, uint32_t* id_i_out) {
+// Reaction lookup, exact radius and symmetric pair draw for the geometric hit (i, j); on success
+// both ends are merged.
+__device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t j, uint32_t d2, uint32_t si, uint32_t t) {
   const DevTables* __restrict__ T = p.tab;
   const uint32_t e = T->rxmap[si * kMaxSpecies + p.oth.sp[j]];
-  if (e == 0xFFu) return kNoKey;
+  if (e == 0xFFu) return;
   const DevRx& rx = T->rx[e];
-  if (d2 > rx.r2) return kNoKey;
+  if (d2 > rx.r2) return;
   const uint32_t id = p.oth.id[i], idj = p.oth.id[j];
   const uint4 r = philox4x32_10(min(id, idj), max(id, idj), t, kTagPair, p.key0, p.key1);
-  if (!fire(r.x, rx.thr)) return kNoKey;
-  *id_i_out = id;
-  return ((unsigned long long)d2 << 32) | idj;
+  if (!fire(r.x, rx.thr)) return;
+  const unsigned long long hi = (unsigned long long)d2 << 32, ki = hi | idj, kj = hi | id;
+  if (atomicMin(&p.best[i], ki) > ki) p.prop[i] = j;
+  if (atomicMin(&p.best[j], kj) > kj) p.prop[j] = i;
+  atomicOr(&p.hasprop[i >> 5], 1u << (i & 31u));
+  atomicOr(&p.hasprop[j >> 5], 1u << (j & 31u));
 }
 
-constexpr int kWarpTaskCap = 256;       // 8 other rows x 32 agents: always fits
+constexpr int kWarpTaskCap = 128;       // 4 forward rows x 32 agents: always fits
 constexpr int kWarpHitCap = 64;
 struct PairWarpSmem {                   // private to one warp
   uint32_t hit_j[kWarpHitCap], hit_d[kWarpHitCap];
-  uint16_t hit_o[kWarpHitCap];          // owner thread | both-directions flag << 15
-  uint16_t task[kWarpTaskCap];          // owner thread | row code (0..8) << 8
+  uint8_t hit_o[kWarpHitCap];           // owner thread
+  uint16_t task[kWarpTaskCap];          // owner thread | row code (5..8) << 8
   uint32_t nhit;
 };
 struct PairSmem {
   int4 pos[kPairThreads];               // x, y, z, species
-  unsigned long long key[kPairThreads];
-  uint32_t row[kPairThreads], xr[kPairThreads], slot[kPairThreads];
+  uint32_t row[kPairThreads], xr[kPairThreads];
   PairWarpSmem w[kPairThreads / 32];
 };
 
-__device__ __forceinline__ void push_hit(PairWarpSmem& W, uint32_t owner, uint32_t j, uint32_t d2, uint32_t both) {
+__device__ __forceinline__ void push_hit(PairWarpSmem& W, uint32_t owner, uint32_t j, uint32_t d2) {
   const uint32_t h = atomicAdd(&W.nhit, 1u);
-  if (h < (uint32_t)kWarpHitCap) { W.hit_j[h] = j; W.hit_d[h] = d2; W.hit_o[h] = (uint16_t)(owner | (both << 15)); }
+  if (h < (uint32_t)kWarpHitCap) { W.hit_j[h] = j; W.hit_d[h] = d2; W.hit_o[h] = (uint8_t)owner; }
 }
 
-// Scan of tile slots [ka, kb) (shared memory) for the agent `owner` at (x, y, z).
-// A hit on a later slot of the owner's own warp stands for both directions of the pair.
+// Tile slots [ka, kb) (shared memory) against the agent `owner` at (x, y, z).
 __device__ __forceinline__ void scan_tile(const Params& p, const PairSmem& S, PairWarpSmem& W, uint32_t ka, uint32_t kb,
                                           uint32_t base, uint32_t owner, int32_t x, int32_t y, int32_t z) {
   const int32_t R = p.max_r;
@@ -347,12 +351,12 @@ __device__ __forceinline__ void scan_tile(const Params& p, const PairSmem& S, Pa
     if (max(max(ux, uy), uz) <= R2) {
       const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (d2 <= p.max_r2) push_hit(W, owner, base + k, d2, (k > owner && k < (owner | 31u) + 1u) ? 1u : 0u);
+      if (d2 <= p.max_r2) push_hit(W, owner, base + k, d2);
     }
   }
 }
 
-// One-direction scan of global slots [j0, j1) for the agent `owner` of the tile at (x, y, z).
+// Global slots [j0, j1) against the agent `owner` of the tile at (x, y, z).
 __device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, uint32_t j0, uint32_t j1, uint32_t owner,
                                             int32_t x, int32_t y, int32_t z) {
   const int32_t R = p.max_r;
@@ -367,40 +371,34 @@ __device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, ui
     if (max(max(ux, uy), uz) <= R2) {
       const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (d2 <= p.max_r2) push_hit(W, owner, j, d2, 0u);
+      if (d2 <= p.max_r2) push_hit(W, owner, j, d2);
     }
   }
 }
 
-// Plain per-thread search of every overlapped row (the definition, as in DESIGN.md §1 phase 2):
-// used for tiles whose hit queue overflowed.
+__device__ __forceinline__ uint32_t row_of(const Params& p, uint32_t rowc, uint32_t c) {
+  return rowc + (uint32_t)(((int32_t)(c % 3u) - 1) * p.nx + ((int32_t)(c / 3u) - 1) * p.nx * p.ny);
+}
+
+// Plain per-thread forward search with immediate merge: used by warps whose hit queue overflowed.
 __device__ __noinline__ void slow_agent(const Params* pp, uint32_t i, int32_t x, int32_t y, int32_t z, uint32_t si,
-                                        uint32_t rowc, uint32_t xlo, uint32_t nxr, uint32_t need, uint32_t t,
-                                        unsigned long long* best_out, uint32_t* slot_out) {
+                                        uint32_t rowc, uint32_t xlo, uint32_t nxr, uint32_t j1_own, uint32_t need, uint32_t t) {
   const Params& p = *pp;
-  unsigned long long best = kNoKey;
-  uint32_t best_j = kNoProp;
   const long long R = p.max_r;
   need |= 1u << 4;
   while (need) {
     const uint32_t c = __ffs(need) - 1u;
     need &= need - 1u;
-    const uint32_t r2 = rowc + (uint32_t)(((int32_t)(c % 3u) - 1) * p.nx + ((int32_t)(c / 3u) - 1) * p.nx * p.ny);
-    const uint32_t j0 = p.cell[r2 + xlo], j1 = p.cell[r2 + xlo + nxr + 1];
+    const uint32_t r2 = row_of(p, rowc, c);
+    const uint32_t j0 = c == 4u ? i + 1u : p.cell[r2 + xlo], j1 = c == 4u ? j1_own : p.cell[r2 + xlo + nxr + 1];
     for (uint32_t j = j0; j < j1; ++j) {
-      if (j == i) continue;
       const long long dx = (long long)p.oth.x[j] - x, dy = (long long)p.oth.y[j] - y, dz = (long long)p.oth.z[j] - z;
       if (dx > R || dx < -R || dy > R || dy < -R || dz > R || dz < -R) continue;
       const unsigned long long d2 = (unsigned long long)(dx * dx + dy * dy + dz * dz);
-      if (d2 > p.max_r2) continue;
-      uint32_t id_i;
-      const unsigned long long k = pair_key(p, i, j, (uint32_t)d2, si, t, &id_i);
-      if (k < best) { best = k; best_j = j; }
+      if (d2 <= p.max_r2) pair_merge(p, i, j, (uint32_t)d2, si, t);
     }
   }
-  *best_out = best; *slot_out = best_j;
 }
-
 
 __global__ void __launch_bounds__(kPairThreads, 6) k_pairs(const __grid_constant__ Params p) {
   __shared__ PairSmem S;
@@ -416,32 +414,27 @@ __global__ void __launch_bounds__(kPairThreads, 6) k_pairs(const __grid_constant
   int32_t x = 0, y = 0, z = 0;
   if (i < n) { s = p.oth.sp[i]; x = p.oth.x[i]; y = p.oth.y[i]; z = p.oth.z[i]; }
   const bool active = s != kDead && ((p.binds_mask >> s) & 1ull);
-  uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0;
+  uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0, j1 = 0;
   if (active) {
     // R <= cell_size (validated), so the R-ball reaches at most one cell further on each side
     const int32_t cx = cell_coord(x, p), cy = cell_coord(y, p), cz = cell_coord(z, p);
     const int32_t lx = x - cx * cs, ly = y - cy * cs, lz = z - cz * cs;
     const uint32_t xm = lx < R && cx > 0, xp = lx >= cs - R && cx < p.nx - 1;
     const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
-    const uint32_t zm = lz < R && cz > 0, zp = lz >= cs - R && cz < p.nz - 1;
+    const uint32_t zp = lz >= cs - R && cz < p.nz - 1;
     xlo = (uint32_t)cx - xm; nxr = xm + xp;
     rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
-    // bit (dz+1)*3 + (dy+1) of `need`: the row at offset (dy, dz) must be searched (bit 4 = own row)
-    const uint32_t ymask = ym | (yp << 2);
-    need = (zm ? (ymask | 2u) : 0u) | (ymask << 3) | (zp ? (ymask | 2u) << 6 : 0u);
+    // forward rows, bit (dz+1)*3 + (dy+1): (y+1, z) = 5; (y-1, z+1), (y, z+1), (y+1, z+1) = 6, 7, 8
+    need = (yp << 5) | (zp ? ((ym | 2u | (yp << 2)) << 6) : 0u);
+    j1 = p.cell[rowc + (uint32_t)cx + xp + 1u];            // end of the own-row forward range, > i
   }
   S.pos[tid] = make_int4(x, y, z, (int32_t)s);
   S.row[tid] = rowc; S.xr[tid] = xlo | (nxr << 30);
-  S.key[tid] = kNoKey; S.slot[tid] = kNoProp;
   __syncthreads();          // the only block-wide barrier: the tile is read-only from here on
 
-  // ---- A: own row
+  // ---- A: own row, slots (i, j1)
   if (active) {
-    const uint32_t j0 = p.cell[rowc + xlo], j1 = p.cell[rowc + xlo + nxr + 1];   // j0 <= i < j1
-    const uint32_t ka = max(j0, base) - base, kb = min(j1, base + kPairThreads) - base, wlo = tid & ~31u;
-    if (ka < wlo) scan_tile(p, S, W, ka, wlo, base, tid, x, y, z);
-    scan_tile(p, S, W, tid + 1u, kb, base, tid, x, y, z);
-    if (j0 < base) scan_global(p, W, j0, base, tid, x, y, z);
+    scan_tile(p, S, W, tid + 1u, min(j1, base + kPairThreads) - base, base, tid, x, y, z);
     if (j1 > base + kPairThreads) scan_global(p, W, base + kPairThreads, j1, tid, x, y, z);
   }
 
@@ -464,13 +457,13 @@ __global__ void __launch_bounds__(kPairThreads, 6) k_pairs(const __grid_constant
   }
   __syncwarp();
 
-  // ---- C: the other rows: 4, 2 or 1 lanes per task
+  // ---- C: the forward rows: 4, 2 or 1 lanes per task
   {
     const uint32_t lg = nt <= 8u ? 2u : (nt <= 16u ? 1u : 0u), items = nt << lg;
     for (uint32_t k = lane; k < items; k += 32u) {
-      const uint32_t e = W.task[k >> lg], c = e >> 8, owner = e & 0xFFu, part = k & ((1u << lg) - 1u);
+      const uint32_t e = W.task[k >> lg], owner = e & 0xFFu, part = k & ((1u << lg) - 1u);
       const uint32_t xr = S.xr[owner], oxlo = xr & 0x3FFFFFFFu, onx = xr >> 30;
-      const uint32_t r2 = S.row[owner] + (uint32_t)(((int32_t)(c % 3u) - 1) * p.nx + ((int32_t)(c / 3u) - 1) * p.nx * p.ny);
+      const uint32_t r2 = row_of(p, S.row[owner], e >> 8);
       const int4 q = S.pos[owner];
       const uint32_t j0 = p.cell[r2 + oxlo], len = p.cell[r2 + oxlo + onx + 1] - j0;
       scan_global(p, W, j0 + ((len * part) >> lg), j0 + ((len * (part + 1u)) >> lg), owner, q.x, q.y, q.z);
@@ -478,50 +471,42 @@ __global__ void __launch_bounds__(kPairThreads, 6) k_pairs(const __grid_constant
   }
   __syncwarp();
 
-  // ---- D: qualify the queued hits and merge them into their owners (all within this warp)
+  // ---- D: qualify the queued hits, one lane per hit
   const uint32_t nh = W.nhit;
   if (nh <= (uint32_t)kWarpHitCap) {
-    for (uint32_t h0 = 0; h0 < nh; h0 += 32u) {      // warp-uniform; one round in the common case
-      const uint32_t h = h0 + lane;
-      unsigned long long k_own = kNoKey, k_oth = kNoKey;
-      uint32_t owner = 0, other = 0, j = 0;
-      if (h < nh) {
-        const uint32_t e = W.hit_o[h];
-        owner = e & 0xFFu; j = W.hit_j[h];
-        uint32_t id_i = 0;
-        k_own = pair_key(p, base + owner, j, W.hit_d[h], (uint32_t)S.pos[owner].w, t, &id_i);
-        if (k_own != kNoKey) {
-          atomicMin(&S.key[owner], k_own);
-          if (e >> 15) {                                   // the partner sees the same pair
-            other = j - base;
-            k_oth = (k_own & 0xFFFFFFFF00000000ull) | id_i;
-            atomicMin(&S.key[other], k_oth);
-          }
-        }
-      }
-      __syncwarp();
-      if (k_own != kNoKey && S.key[owner] == k_own) S.slot[owner] = j;            // keys are unique per owner
-      if (k_oth != kNoKey && S.key[other] == k_oth) S.slot[other] = base + owner;
-      __syncwarp();
+    for (uint32_t h = lane; h < nh; h += 32u) {
+      const uint32_t owner = W.hit_o[h];
+      pair_merge(p, base + owner, W.hit_j[h], W.hit_d[h], (uint32_t)S.pos[owner].w, t);
     }
   } else if (active) {
-    unsigned long long kb; uint32_t sb;
-    slow_agent(&p, i, x, y, z, s, rowc, xlo, nxr, need, t, &kb, &sb);
-    S.key[tid] = kb; S.slot[tid] = sb;
+    slow_agent(&p, i, x, y, z, s, rowc, xlo, nxr, j1, need, t);
   }
-  __syncwarp();
-  const bool found = S.key[tid] != kNoKey;
-  const uint32_t word = __ballot_sync(0xFFFFFFFFu, found);
-  if (lane == 0 && base + warp * 32u < n) p.hasprop[(base >> 5) + warp] = word;
-  if (found) p.prop[i] = S.slot[tid];
 }
 
 // ----------------------------------------------------------------------------- K4b handshake resolve
 // Phase 2b: a binding happens iff the proposal is mutual (a7).  One thread per word of the hasprop
 // bitmap; the lower slot of a mutual pair rewrites both species in place (anchor -> complex, the
 // other -> DEAD; S10).  No other thread reads or writes the species of a matched agent in this
-// kernel: a third agent that proposed to one of them only reads prop[].
-__global__ void __launch_bounds__(256) k_resolve(Params p) {
+// kernel: a third agent that proposed to one of them only reads best[] / bslot[].
+
+// Slot of the agent with id `idj` at squared distance d2 from agent i (it exists): the plain
+// neighbourhood sweep, used only when bslot[i] lost a store race (see K4, D).
+__device__ __noinline__ uint32_t find_partner(const Params* pp, uint32_t i, uint32_t idj) {
+  const Params& p = *pp;
+  const int32_t x = p.oth.x[i], y = p.oth.y[i], z = p.oth.z[i], R = p.max_r;
+  const int32_t xlo = cell_coord(max(x - R, 0), p), xhi = min(cell_coord(x + R, p), p.nx - 1);
+  const int32_t ylo = cell_coord(max(y - R, 0), p), yhi = min(cell_coord(y + R, p), p.ny - 1);
+  const int32_t zlo = cell_coord(max(z - R, 0), p), zhi = min(cell_coord(z + R, p), p.nz - 1);
+  for (int32_t cz = zlo; cz <= zhi; ++cz)
+    for (int32_t cy = ylo; cy <= yhi; ++cy) {
+      const uint32_t rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
+      for (uint32_t j = p.cell[rowc + xlo]; j < p.cell[rowc + xhi + 1]; ++j)
+        if (p.oth.id[j] == idj) return j;
+    }
+  return kNoProp;
+}
+
+__global__ void __launch_bounds__(256) k_resolve(const __grid_constant__ Params p) {
   __shared__ int32_t s_delta[kMaxRowWidth];
   delta_zero(s_delta, p.row_width);
   const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
@@ -532,12 +517,16 @@ __global__ void __launch_bounds__(256) k_resolve(Params p) {
     while (bits) {
       const uint32_t b = __ffs(bits) - 1u;
       bits &= bits - 1u;
-      const uint32_t i = w * 32u + b, j = p.prop[i];
+      const uint32_t i = w * 32u + b;
+      const uint32_t idj = (uint32_t)p.best[i];            // low word of (d2, id of the proposed partner)
+      uint32_t j = p.prop[i];
+      if (j >= n || p.oth.id[j] != idj) j = find_partner(&p, i, idj);
       if (j <= i) continue;                                   // the lower slot handles the pair
-      if (!((p.hasprop[j >> 5] >> (j & 31u)) & 1u) || p.prop[j] != i) continue;
+      const uint32_t idi = p.oth.id[i];
+      if ((uint32_t)p.best[j] != idi) continue;               // not mutual (best[j] = kNoKey if j never proposed)
       const uint16_t si = p.oth.sp[i], sj = p.oth.sp[j];
       const DevRx& rx = T->rx[T->rxmap[(uint32_t)si * kMaxSpecies + sj]];
-      const bool anchor_i = (si != sj) ? (si == rx.a) : (p.oth.id[i] < p.oth.id[j]);
+      const bool anchor_i = (si != sj) ? (si == rx.a) : (idi < idj);
       p.oth.sp[i] = anchor_i ? rx.cplx : kDead;
       p.oth.sp[j] = anchor_i ? kDead : rx.cplx;
       int32_t* d = s_delta + ((uint32_t)p.oth.x[i] >> p.stride_shift) * p.n_species;
@@ -721,7 +710,7 @@ __global__ void __launch_bounds__(128) k_births(Params p) {
 }
 
 // ----------------------------------------------------------------------------- K7 epilogue
-// Clears the touched bitmap words; the last block to finish advances the device scalars and
+// Clears the touched birth-bitmap words and proposal entries; the last block to finish advances the device scalars and
 // seeds counts row t+2 with row t+1 (the next step adds its deltas to it; a10).
 __global__ void __launch_bounds__(256) k_epilogue(Params p) {
   __shared__ uint32_t s_last;
@@ -730,6 +719,18 @@ __global__ void __launch_bounds__(256) k_epilogue(Params p) {
   for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < nb; e += stride) {
     const uint32_t pid = p.oth.id[p.birth_list[e].x];
     p.bits[pid >> 3] = 0u;
+  }
+  // proposals of this step: back to "none" (only the touched entries) for the next step's K4
+  const uint32_t nw = (p.cell[p.n_cells] + 31u) >> 5;
+  for (uint32_t w = blockIdx.x * blockDim.x + threadIdx.x; w < nw; w += stride) {
+    uint32_t bits = p.hasprop[w];
+    if (!bits) continue;
+    p.hasprop[w] = 0u;
+    while (bits) {
+      const uint32_t b = __ffs(bits) - 1u;
+      bits &= bits - 1u;
+      p.best[w * 32u + b] = kNoKey;
+    }
   }
   __threadfence();
   __syncthreads();

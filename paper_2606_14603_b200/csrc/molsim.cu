@@ -27,7 +27,7 @@ const char* kKernelNames[SIM_N_KERNELS] = {
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t soa[2][5], off, prop, hasprop, cell, partial, bits, chunk_prefix, birth_list, counts,
+  size_t soa[2][5], off, prop, best, hasprop, cell, partial, bits, chunk_prefix, birth_list, counts,
       scal, tab, gauss, total;
   uint32_t n_cells, nx, ny, nz;
 };
@@ -43,6 +43,7 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   const size_t cap = c->capacity;
   for (int b = 0; b < 2; ++b) for (int a = 0; a < 5; ++a) L.soa[b][a] = take(cap * (a < 4 ? 4 : 2) + 64);
   L.off = take(cap * 4); L.prop = take(cap * 4);
+  L.best = take(cap * 8);
   L.hasprop = take((cap / 32 + 16) * 4);
   L.cell = take(((size_t)nc + 1 + 1024) * 4);
   L.partial = take(4096 * 4);
@@ -301,6 +302,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
                                      (uint16_t*)(w + L.soa[b][4])}; };
   p.cur = soa(0); p.oth = soa(1);
   p.off = (uint32_t*)(w + L.off); p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
+  p.best = (unsigned long long*)(w + L.best);
   p.cell = (uint32_t*)(w + L.cell); p.partial = (uint32_t*)(w + L.partial);
   p.bits = (uint32_t*)(w + L.bits); p.chunk_prefix = (uint32_t*)(w + L.chunk_prefix);
   p.birth_list = (uint2*)(w + L.birth_list); p.counts = (uint32_t*)(w + L.counts);
@@ -360,6 +362,8 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   for (int r = 0; r < kMaxRules; ++r) sc.t_first[r] = kNever;
   bool ok = true;
   ok = ok && cudaMemsetAsync(p.bits, 0, L.chunk_prefix - L.bits, s->stream) == cudaSuccess;
+  ok = ok && cudaMemsetAsync(p.best, 0xFF, L.hasprop - L.best, s->stream) == cudaSuccess;
+  ok = ok && cudaMemsetAsync(p.hasprop, 0, L.cell - L.hasprop, s->stream) == cudaSuccess;
   ok = ok && cudaMemsetAsync(p.counts, 0, L.scal - L.counts, s->stream) == cudaSuccess;
   ok = ok && cudaMemcpyAsync(p.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream) == cudaSuccess;
   ok = ok && cudaMemcpyAsync((void*)p.tab, &T, sizeof(T), cudaMemcpyHostToDevice, s->stream) == cudaSuccess;
