@@ -65,7 +65,7 @@ struct Params {
   uint32_t* off;            // within-cell rank from the histogram pass
   unsigned long long* best; // proposal key (dist^2 << 32 | partner id) per sorted slot, ~0 = none
   uint32_t* prop;           // slot of the partner that last lowered best[i] (checked against the key in K4b)
-  uint32_t* hasprop;        // 1 bit per sorted slot: best[i] was touched this step (cleared by K7)
+  uint32_t* hasprop;        // 1 bit per sorted slot: best[i] was touched this step (cleared by K5)
   uint32_t* cell;           // [n_cells + 1]: counts, then exclusive starts; cell[n_cells] = n_sorted
   uint32_t* partial;        // scan partials
   uint32_t* bits;           // birth bitmap, 4 bits per id

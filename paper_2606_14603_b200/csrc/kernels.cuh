@@ -1,7 +1,7 @@
 // kernels.cuh — the hand-written sm_100a kernels of the molecule-agent step.
 // Product code (CUDA path).  Shares nothing with oracle/.
 //
-// One step = K1 move+hist -> K2 cell scan (2 launches) -> K3 scatter -> K4 pair search/proposal ->
+// One step = K1 move+hist -> K2 cell scan (2 launches) -> K3 move+scatter -> K4 pair search/proposal ->
 // K4b resolve -> K5 unimolecular -> K6 birth scan (2 launches) + birth placement -> K7 epilogue.
 // Every decision is keyed by agent id (never by slot), so the nondeterministic slot order the
 // histogram atomics produce inside a cell cannot change any result.
@@ -69,32 +69,59 @@ __device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* s_warp /*[9]
 }
 
 // ----------------------------------------------------------------------------- K1 move + histogram
-// Phase 1 (Brownian move, boundary and compartment rule) fused with the cell-key histogram of the
-// counting sort.  Gaussian inverse-CDF tables are staged in shared memory.
+// Phase 1 (Brownian move, boundary and compartment rule) is a pure function of
+// (species, position, id, t): move_agent() below.  K1 evaluates it only to get the cell key for the
+// histogram of the counting sort (a3) and stores nothing but the within-cell rank; K3 evaluates it
+// again while it scatters, so the moved positions are written once, at their sorted slot, and the
+// 12 B/agent write + re-read of an in-place move never happens (a second Philox is cheaper).
+struct Moved { int32_t x, y, z; uint16_t s; };
+
+__device__ __forceinline__ Moved move_agent(const Params& p, const DevTables* __restrict__ T, const int16_t* g,
+                                            uint16_t s, int32_t x, int32_t y, int32_t z, uint32_t id, uint32_t t) {
+  Moved m{x, y, z, s};
+  const DevSpecies& S = T->sp[s];
+  const uint32_t cls = S.sigma_class;
+  if (!cls) return m;
+  const uint32_t sh = 32u - p.table_bits;
+  const uint4 r = philox4x32_10(id, 0u, t, kTagMove, p.key0, p.key1);
+  const int16_t* tb = g + (cls << p.table_bits);
+  const int32_t rbase = (int32_t)(((uint32_t)x >> p.stride_shift) << p.stride_shift);
+  int32_t qx = x - rbase + tb[r.x >> sh], qy = y + tb[r.y >> sh], qz = z + tb[r.z >> sh];
+  const DevComp& c = T->comp[S.compartment];
+  if (c.shape == 0) {
+    qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L);
+  } else if (!comp_valid(c, qx, qy, qz)) {
+    const uint16_t ct = S.cross_to;
+    if (ct != kDead && comp_valid(T->comp[T->sp[ct].compartment], qx, qy, qz) && fire(r.w, S.cross_thr)) m.s = ct;
+    else return m;                       // no-flux wall: the agent keeps its position (S6)
+  }
+  m.x = qx + rbase; m.y = qy; m.z = qz;
+  return m;
+}
+
+// Gaussian inverse-CDF tables are staged in shared memory (north_star (2)).
+__device__ __forceinline__ const int16_t* stage_gauss(const Params& p, int16_t* s_gauss, int gauss_in_smem) {
+  if (!gauss_in_smem) return p.gauss;
+  const uint32_t n_tab = p.n_classes << p.table_bits;
+  for (uint32_t k = threadIdx.x; k < n_tab; k += blockDim.x) s_gauss[k] = p.gauss[k];
+  __syncthreads();
+  return s_gauss;
+}
+
 // A block walks tiles of 256 x kMoveUnroll agents; every thread keeps kMoveUnroll agents in flight
 // (all loads issued before the first Philox, all histogram atomics before the first rank store) so
 // that HBM and L2-atomic latency overlap.  The histogram uses warp-aggregated atomics
 // (__match_any_sync on the cell key): agents arrive nearly cell-sorted from the previous step, so a
-// warp touches few distinct cells.  Counts deltas for membrane crossings go straight to counts
-// row t+1 (rare events).
+// warp touches few distinct cells.
 constexpr int kMoveUnroll = 4;
 constexpr int kMoveThreads = 256;
 
-template <bool kHist>
 __global__ void __launch_bounds__(kMoveThreads) k_move_hist(Params p, int gauss_in_smem) {
   extern __shared__ int16_t s_gauss[];
-  const int16_t* g = p.gauss;
-  if (gauss_in_smem) {
-    const uint32_t n_tab = p.n_classes << p.table_bits;
-    for (uint32_t k = threadIdx.x; k < n_tab; k += blockDim.x) s_gauss[k] = p.gauss[k];
-    __syncthreads();
-    g = s_gauss;
-  }
+  const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   const DevTables* __restrict__ T = p.tab;
-  const uint32_t sh = 32u - p.table_bits;
   const uint32_t lane = threadIdx.x & 31u;
-  uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
   constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {   // block-uniform trip count
     uint16_t s[kMoveUnroll];
@@ -114,53 +141,37 @@ __global__ void __launch_bounds__(kMoveThreads) k_move_hist(Params p, int gauss_
     for (int a = 0; a < kMoveUnroll; ++a) {
       key[a] = 0xFFFFFFFFu;
       if (s[a] == kDead) continue;
-      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
-      const DevSpecies& S = T->sp[s[a]];
-      const uint32_t cls = S.sigma_class;
-      if (cls) {
-        const uint4 r = philox4x32_10(id[a], 0u, t, kTagMove, p.key0, p.key1);
-        const int16_t* tb = g + (cls << p.table_bits);
-        const int32_t rbase = (int32_t)(((uint32_t)x[a] >> p.stride_shift) << p.stride_shift);
-        int32_t qx = x[a] - rbase + tb[r.x >> sh], qy = y[a] + tb[r.y >> sh], qz = z[a] + tb[r.z >> sh];
-        const DevComp& c = T->comp[S.compartment];
-        bool accept = true;
-        if (c.shape == 0) {
-          qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L);
-        } else if (!comp_valid(c, qx, qy, qz)) {
-          accept = false;
-          const uint16_t ct = S.cross_to;
-          if (ct != kDead && comp_valid(T->comp[T->sp[ct].compartment], qx, qy, qz) && fire(r.w, S.cross_thr)) {
-            accept = true;
-            p.cur.sp[i] = ct;
-            const uint32_t rep = (uint32_t)x[a] >> p.stride_shift;
-            atomicSub(&row[rep * p.n_species + s[a]], 1u);
-            atomicAdd(&row[rep * p.n_species + ct], 1u);
-          }
-        }
-        if (accept) {
-          x[a] = qx + rbase; y[a] = qy; z[a] = qz;
-          p.cur.x[i] = x[a]; p.cur.y[i] = y[a]; p.cur.z[i] = z[a];
-        }
-      }
-      if (kHist) key[a] = cell_key(x[a], y[a], z[a], p);
+      const Moved m = move_agent(p, T, g, s[a], x[a], y[a], z[a], id[a], t);
+      key[a] = cell_key(m.x, m.y, m.z, p);
     }
-    if (kHist) {
-      uint32_t first[kMoveUnroll], rank[kMoveUnroll];
-      int leader[kMoveUnroll];
+    uint32_t first[kMoveUnroll], rank[kMoveUnroll];
+    int leader[kMoveUnroll];
 #pragma unroll
-      for (int a = 0; a < kMoveUnroll; ++a) {
-        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key[a]);
-        leader[a] = __ffs(peers) - 1;
-        rank[a] = __popc(peers & ((1u << lane) - 1u));
-        first[a] = 0;
-        if (s[a] != kDead && (int)lane == leader[a]) first[a] = atomicAdd(&p.cell[key[a]], (uint32_t)__popc(peers));
-      }
-#pragma unroll
-      for (int a = 0; a < kMoveUnroll; ++a) {
-        const uint32_t f = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]);
-        if (s[a] != kDead) p.off[base + a * kMoveThreads + threadIdx.x] = f + rank[a];
-      }
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key[a]);
+      leader[a] = __ffs(peers) - 1;
+      rank[a] = __popc(peers & ((1u << lane) - 1u));
+      first[a] = 0;
+      if (s[a] != kDead && (int)lane == leader[a]) first[a] = atomicAdd(&p.cell[key[a]], (uint32_t)__popc(peers));
     }
+#pragma unroll
+    for (int a = 0; a < kMoveUnroll; ++a) {
+      const uint32_t f = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]);
+      if (s[a] != kDead) p.off[base + a * kMoveThreads + threadIdx.x] = f + rank[a];
+    }
+  }
+}
+
+// Test hook (sim_debug_move_only): phase 1 in place on the current arrays.
+__global__ void __launch_bounds__(kMoveThreads) k_move_only(Params p, int gauss_in_smem) {
+  extern __shared__ int16_t s_gauss[];
+  const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
+  const uint32_t n = p.scal->n_slots, t = p.scal->t;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const uint16_t s = p.cur.sp[i];
+    if (s == kDead) continue;
+    const Moved m = move_agent(p, p.tab, g, s, p.cur.x[i], p.cur.y[i], p.cur.z[i], p.cur.id[i], t);
+    p.cur.x[i] = m.x; p.cur.y[i] = m.y; p.cur.z[i] = m.z; p.cur.sp[i] = m.s;
   }
 }
 
@@ -216,12 +227,18 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
   if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) cell[n] = running;   // = number of live agents
 }
 
-// ----------------------------------------------------------------------------- K3 scatter / reorder
-// Counting-sort scatter that reorders the whole structure of arrays into cell order (a5) and drops
-// DEAD slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
-// kMoveUnroll agents in flight per thread.
-__global__ void __launch_bounds__(kMoveThreads) k_scatter(Params p) {
-  const uint32_t n = p.scal->n_slots;
+// ----------------------------------------------------------------------------- K3 move + scatter / reorder
+// Counting-sort scatter that reorders the whole structure of arrays into cell order (a5), applying
+// phase 1 on the way (move_agent again: same result as in K1, so the same cell), and drops DEAD
+// slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
+// kMoveUnroll agents in flight per thread.  Membrane crossings change the species here; their
+// counts deltas go straight to counts row t+1 (rare events).
+__global__ void __launch_bounds__(kMoveThreads) k_scatter(Params p, int gauss_in_smem) {
+  extern __shared__ int16_t s_gauss[];
+  const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
+  const uint32_t n = p.scal->n_slots, t = p.scal->t;
+  const DevTables* __restrict__ T = p.tab;
+  uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
   constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {
     uint16_t s[kMoveUnroll];
@@ -241,7 +258,15 @@ __global__ void __launch_bounds__(kMoveThreads) k_scatter(Params p) {
     }
 #pragma unroll
     for (int a = 0; a < kMoveUnroll; ++a) {
-      if (s[a] != kDead) off[a] += p.cell[cell_key(x[a], y[a], z[a], p)];
+      if (s[a] == kDead) continue;
+      const Moved m = move_agent(p, T, g, s[a], x[a], y[a], z[a], id[a], t);
+      if (m.s != s[a]) {
+        const uint32_t rep = (uint32_t)x[a] >> p.stride_shift;
+        atomicSub(&row[rep * p.n_species + s[a]], 1u);
+        atomicAdd(&row[rep * p.n_species + m.s], 1u);
+      }
+      x[a] = m.x; y[a] = m.y; z[a] = m.z; s[a] = m.s;
+      off[a] += p.cell[cell_key(m.x, m.y, m.z, p)];
     }
 #pragma unroll
     for (int a = 0; a < kMoveUnroll; ++a) {
@@ -538,9 +563,10 @@ __global__ void __launch_bounds__(256) k_resolve(const __grid_constant__ Params 
 
 // ----------------------------------------------------------------------------- K5 unimolecular
 // Phase 3 (a8): per agent, per channel, Philox(seed, t, id) word < threshold.  Most agents belong to
-// a species without channels: a thread reads the species of 8 agents with one 128-bit load and
-// touches id / position only for those that have channels (chan_mask).  Species are rewritten in
-// place only where they change.  Firing parents are appended to the birth list and flagged in the
+// a species without channels: a thread reads the species of 8 agents with one 128-bit load; the
+// slots of those that have channels (chan_mask) are compacted into a shared list and only these
+// are processed, one per thread, so the Philox work is dense.  Species are rewritten in place only
+// where they change.  The same pass clears the proposal state K4 left (hasprop byte -> best[]).  Firing parents are appended to the birth list and flagged in the
 // id-indexed birth bitmap (4 bits per id) that K6 ranks.  Counts deltas are block-aggregated.
 __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __restrict__ T, uint32_t i, uint16_t s0,
                                         uint32_t t, int32_t* s_delta) {
@@ -591,14 +617,20 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
   }
 }
 
-__global__ void __launch_bounds__(256) k_uni(Params p) {
+constexpr int kUniThreads = 256;
+constexpr int kUniTile = kUniThreads * 8;
+__global__ void __launch_bounds__(kUniThreads) k_uni(Params p) {
   __shared__ int32_t s_delta[kMaxRowWidth];
+  __shared__ uint16_t s_list[kUniTile];      // tile-local slots of the agents that have channels
+  __shared__ uint32_t s_n;
   delta_zero(s_delta, p.row_width);
   const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
   const DevTables* __restrict__ T = p.tab;
-  const uint32_t ng = (n + 7u) >> 3;
-  for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
-    const uint32_t i0 = g * 8u;
+  const uint32_t lane = threadIdx.x & 31u;
+  for (uint32_t base = blockIdx.x * kUniTile; base < n; base += gridDim.x * kUniTile) {   // block-uniform
+    if (threadIdx.x == 0) s_n = 0;
+    __syncthreads();
+    const uint32_t l0 = threadIdx.x * 8u, i0 = base + l0;
     uint32_t w[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
     if (i0 + 8u <= n) {
       const uint4 q = *reinterpret_cast<const uint4*>(p.oth.sp + i0);
@@ -609,12 +641,45 @@ __global__ void __launch_bounds__(256) k_uni(Params p) {
         w[k >> 1] = (k & 1u) ? ((w[k >> 1] & 0x0000FFFFu) | (v << 16)) : ((w[k >> 1] & 0xFFFF0000u) | v);
       }
     }
+    // this step's proposals are resolved: put the touched best[] entries back to "none" for the next K4
+    if (i0 < n) {
+      uint8_t* hp = reinterpret_cast<uint8_t*>(p.hasprop) + (i0 >> 3);
+      uint32_t bits = *hp;
+      if (bits) {
+        *hp = 0;
+        while (bits) { p.best[i0 + __ffs(bits) - 1u] = kNoKey; bits &= bits - 1u; }
+      }
+    }
+    uint32_t mask = 0;
 #pragma unroll
     for (uint32_t k = 0; k < 8u; ++k) {
       const uint32_t s = (w[k >> 1] >> ((k & 1u) * 16u)) & 0xFFFFu;
-      if (s == kDead || !((p.chan_mask >> s) & 1ull)) continue;
-      uni_one(p, T, i0 + k, (uint16_t)s, t, s_delta);
+      if (s != kDead && ((p.chan_mask >> s) & 1ull)) mask |= 1u << k;
     }
+    // compact: warp-inclusive scan of the counts, one shared atomic per warp
+    const uint32_t cnt = __popc(mask);
+    uint32_t incl = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+      if (lane >= (uint32_t)d) incl += o;
+    }
+    const uint32_t wtotal = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    uint32_t wbase = 0;
+    if (lane == 31 && wtotal) wbase = atomicAdd(&s_n, wtotal);
+    wbase = __shfl_sync(0xFFFFFFFFu, wbase, 31);
+    uint32_t pos = wbase + incl - cnt;
+    while (mask) {
+      s_list[pos++] = (uint16_t)(l0 + __ffs(mask) - 1u);
+      mask &= mask - 1u;
+    }
+    __syncthreads();
+    const uint32_t m = s_n;
+    for (uint32_t k = threadIdx.x; k < m; k += kUniThreads) {
+      const uint32_t i = base + s_list[k];
+      uni_one(p, T, i, p.oth.sp[i], t, s_delta);
+    }
+    __syncthreads();   // s_list / s_n are reused by the next tile
   }
   delta_flush(s_delta, p.counts + (size_t)(t + 1) * p.row_width, p.row_width);
 }
@@ -710,7 +775,7 @@ __global__ void __launch_bounds__(128) k_births(Params p) {
 }
 
 // ----------------------------------------------------------------------------- K7 epilogue
-// Clears the touched birth-bitmap words and proposal entries; the last block to finish advances the device scalars and
+// Clears the touched birth-bitmap words; the last block to finish advances the device scalars and
 // seeds counts row t+2 with row t+1 (the next step adds its deltas to it; a10).
 __global__ void __launch_bounds__(256) k_epilogue(Params p) {
   __shared__ uint32_t s_last;
@@ -719,18 +784,6 @@ __global__ void __launch_bounds__(256) k_epilogue(Params p) {
   for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < nb; e += stride) {
     const uint32_t pid = p.oth.id[p.birth_list[e].x];
     p.bits[pid >> 3] = 0u;
-  }
-  // proposals of this step: back to "none" (only the touched entries) for the next step's K4
-  const uint32_t nw = (p.cell[p.n_cells] + 31u) >> 5;
-  for (uint32_t w = blockIdx.x * blockDim.x + threadIdx.x; w < nw; w += stride) {
-    uint32_t bits = p.hasprop[w];
-    if (!bits) continue;
-    p.hasprop[w] = 0u;
-    while (bits) {
-      const uint32_t b = __ffs(bits) - 1u;
-      bits &= bits - 1u;
-      p.best[w * 32u + b] = kNoKey;
-    }
   }
   __threadfence();
   __syncthreads();
