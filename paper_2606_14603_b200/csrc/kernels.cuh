@@ -113,10 +113,16 @@ __device__ __forceinline__ const int16_t* stage_gauss(const Params& p, int16_t* 
 // that HBM and L2-atomic latency overlap.  The histogram uses warp-aggregated atomics
 // (__match_any_sync on the cell key): agents arrive nearly cell-sorted from the previous step, so a
 // warp touches few distinct cells.
-constexpr int kMoveUnroll = 4;
+#ifndef MOLSIM_MOVE_UNROLL
+#define MOLSIM_MOVE_UNROLL 2     // tuned on B200 (W4 16M): 2 agents in flight per thread x 5 blocks/SM
+#endif
+#ifndef MOLSIM_MOVE_MINBLK
+#define MOLSIM_MOVE_MINBLK 5
+#endif
+constexpr int kMoveUnroll = MOLSIM_MOVE_UNROLL;
 constexpr int kMoveThreads = 256;
 
-__global__ void __launch_bounds__(kMoveThreads) k_move_hist(Params p, int gauss_in_smem) {
+__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(Params p, int gauss_in_smem) {
   extern __shared__ int16_t s_gauss[];
   const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
@@ -233,7 +239,7 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
 // slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
 // kMoveUnroll agents in flight per thread.  Membrane crossings change the species here; their
 // counts deltas go straight to counts row t+1 (rare events).
-__global__ void __launch_bounds__(kMoveThreads) k_scatter(Params p, int gauss_in_smem) {
+__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_scatter(Params p, int gauss_in_smem) {
   extern __shared__ int16_t s_gauss[];
   const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
