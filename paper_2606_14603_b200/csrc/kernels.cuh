@@ -76,36 +76,56 @@ __device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* s_warp /*[9]
 // 12 B/agent write + re-read of an in-place move never happens (a second Philox is cheaper).
 struct Moved { int32_t x, y, z; uint16_t s; };
 
-__device__ __forceinline__ Moved move_agent(const Params& p, const DevTables* __restrict__ T, const int16_t* g,
+// What phase 1 needs of the tables, staged in shared memory next to the Gaussian tables so that
+// the move never waits on a chain of dependent global loads.
+struct SpLite { uint8_t cls, comp; uint16_t cross_to; uint32_t cross_thr; };
+struct MoveTables {
+  SpLite sp[kMaxSpecies];
+  DevComp comp[kMaxCompartments];
+};
+
+__device__ __forceinline__ Moved move_agent(const Params& p, const MoveTables& M, const int16_t* g,
                                             uint16_t s, int32_t x, int32_t y, int32_t z, uint32_t id, uint32_t t) {
   Moved m{x, y, z, s};
-  const DevSpecies& S = T->sp[s];
-  const uint32_t cls = S.sigma_class;
+  const SpLite S = M.sp[s];
+  const uint32_t cls = S.cls;
   if (!cls) return m;
   const uint32_t sh = 32u - p.table_bits;
   const uint4 r = philox4x32_10(id, 0u, t, kTagMove, p.key0, p.key1);
   const int16_t* tb = g + (cls << p.table_bits);
   const int32_t rbase = (int32_t)(((uint32_t)x >> p.stride_shift) << p.stride_shift);
   int32_t qx = x - rbase + tb[r.x >> sh], qy = y + tb[r.y >> sh], qz = z + tb[r.z >> sh];
-  const DevComp& c = T->comp[S.compartment];
+  const DevComp& c = M.comp[S.comp];
   if (c.shape == 0) {
     qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L);
   } else if (!comp_valid(c, qx, qy, qz)) {
     const uint16_t ct = S.cross_to;
-    if (ct != kDead && comp_valid(T->comp[T->sp[ct].compartment], qx, qy, qz) && fire(r.w, S.cross_thr)) m.s = ct;
+    if (ct != kDead && comp_valid(M.comp[M.sp[ct].comp], qx, qy, qz) && fire(r.w, S.cross_thr)) m.s = ct;
     else return m;                       // no-flux wall: the agent keeps its position (S6)
   }
   m.x = qx + rbase; m.y = qy; m.z = qz;
   return m;
 }
 
-// Gaussian inverse-CDF tables are staged in shared memory (north_star (2)).
-__device__ __forceinline__ const int16_t* stage_gauss(const Params& p, int16_t* s_gauss, int gauss_in_smem) {
-  if (!gauss_in_smem) return p.gauss;
-  const uint32_t n_tab = p.n_classes << p.table_bits;
-  for (uint32_t k = threadIdx.x; k < n_tab; k += blockDim.x) s_gauss[k] = p.gauss[k];
+// Gaussian inverse-CDF tables (north_star (2)) and the species / compartment fields are staged in
+// shared memory once per (persistent) block.
+__device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTables& M, int16_t* s_gauss, int gauss_in_smem) {
+  const DevTables* __restrict__ T = p.tab;
+  for (uint32_t k = threadIdx.x; k < (uint32_t)kMaxSpecies; k += blockDim.x) {
+    const DevSpecies& S = T->sp[k];
+    M.sp[k] = SpLite{S.sigma_class, S.compartment, S.cross_to, S.cross_thr};
+  }
+  for (uint32_t k = threadIdx.x; k < (uint32_t)kMaxCompartments; k += blockDim.x) M.comp[k] = T->comp[k];
+  const int16_t* g = p.gauss;
+  if (gauss_in_smem) {
+    const uint32_t n_words = (p.n_classes << p.table_bits) >> 1;      // table_bits >= 1: an even number of int16
+    const uint32_t* src = reinterpret_cast<const uint32_t*>(p.gauss);
+    uint32_t* dst = reinterpret_cast<uint32_t*>(s_gauss);
+    for (uint32_t k = threadIdx.x; k < n_words; k += blockDim.x) dst[k] = src[k];
+    g = s_gauss;
+  }
   __syncthreads();
-  return s_gauss;
+  return g;
 }
 
 // A block walks tiles of 256 x kMoveUnroll agents; every thread keeps kMoveUnroll agents in flight
@@ -123,10 +143,10 @@ constexpr int kMoveUnroll = MOLSIM_MOVE_UNROLL;
 constexpr int kMoveThreads = 256;
 
 __global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(Params p, int gauss_in_smem) {
-  extern __shared__ int16_t s_gauss[];
-  const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
+  extern __shared__ __align__(16) int16_t s_gauss[];
+  __shared__ MoveTables M;
+  const int16_t* g = stage_tables(p, M, s_gauss, gauss_in_smem);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
-  const DevTables* __restrict__ T = p.tab;
   const uint32_t lane = threadIdx.x & 31u;
   constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {   // block-uniform trip count
@@ -141,13 +161,13 @@ __global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(
 #pragma unroll
     for (int a = 0; a < kMoveUnroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
-      if (s[a] != kDead) { x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; }
+      if (i < n) { x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; }   // not gated on the species: one round trip
     }
 #pragma unroll
     for (int a = 0; a < kMoveUnroll; ++a) {
       key[a] = 0xFFFFFFFFu;
       if (s[a] == kDead) continue;
-      const Moved m = move_agent(p, T, g, s[a], x[a], y[a], z[a], id[a], t);
+      const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
       key[a] = cell_key(m.x, m.y, m.z, p);
     }
     uint32_t first[kMoveUnroll], rank[kMoveUnroll];
@@ -170,13 +190,14 @@ __global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(
 
 // Test hook (sim_debug_move_only): phase 1 in place on the current arrays.
 __global__ void __launch_bounds__(kMoveThreads) k_move_only(Params p, int gauss_in_smem) {
-  extern __shared__ int16_t s_gauss[];
-  const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
+  extern __shared__ __align__(16) int16_t s_gauss[];
+  __shared__ MoveTables M;
+  const int16_t* g = stage_tables(p, M, s_gauss, gauss_in_smem);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const uint16_t s = p.cur.sp[i];
     if (s == kDead) continue;
-    const Moved m = move_agent(p, p.tab, g, s, p.cur.x[i], p.cur.y[i], p.cur.z[i], p.cur.id[i], t);
+    const Moved m = move_agent(p, M, g, s, p.cur.x[i], p.cur.y[i], p.cur.z[i], p.cur.id[i], t);
     p.cur.x[i] = m.x; p.cur.y[i] = m.y; p.cur.z[i] = m.z; p.cur.sp[i] = m.s;
   }
 }
@@ -240,10 +261,10 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
 // kMoveUnroll agents in flight per thread.  Membrane crossings change the species here; their
 // counts deltas go straight to counts row t+1 (rare events).
 __global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_scatter(Params p, int gauss_in_smem) {
-  extern __shared__ int16_t s_gauss[];
-  const int16_t* g = stage_gauss(p, s_gauss, gauss_in_smem);
+  extern __shared__ __align__(16) int16_t s_gauss[];
+  __shared__ MoveTables M;
+  const int16_t* g = stage_tables(p, M, s_gauss, gauss_in_smem);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
-  const DevTables* __restrict__ T = p.tab;
   uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
   constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {
@@ -258,14 +279,14 @@ __global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_scatter(Pa
 #pragma unroll
     for (int a = 0; a < kMoveUnroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
-      if (s[a] != kDead) {
+      if (i < n) {   // not gated on the species: one round trip
         x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; off[a] = p.off[i];
       }
     }
 #pragma unroll
     for (int a = 0; a < kMoveUnroll; ++a) {
       if (s[a] == kDead) continue;
-      const Moved m = move_agent(p, T, g, s[a], x[a], y[a], z[a], id[a], t);
+      const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
       if (m.s != s[a]) {
         const uint32_t rep = (uint32_t)x[a] >> p.stride_shift;
         atomicSub(&row[rep * p.n_species + s[a]], 1u);
