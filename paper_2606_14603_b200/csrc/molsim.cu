@@ -136,7 +136,12 @@ struct sim {
   Layout lay;
   Params prm;         // prm.cur / prm.oth always describe the CURRENT parity
   char* ws = nullptr;
-  cudaStream_t stream = nullptr;
+  cudaStream_t stream = nullptr;   // the caller's stream: everything executes here
+  cudaStream_t run = nullptr;      // where enqueue_step puts its launches: `stream`, or `cap` while a graph is captured
+  cudaStream_t cap = nullptr;      // private stream used only to CAPTURE the step graphs (never executes work)
+  cudaGraphExec_t g1[2] = {nullptr, nullptr}, g8[2] = {nullptr, nullptr};   // 1 / 8 steps, by starting parity
+  bool graphs_tried = false, graphs_ok = false;
+  uint32_t kernels_per_step = 0;
   uint32_t t_host = 0;           // steps enqueued so far (the host knows t exactly)
   uint64_t launches = 0;
   int gauss_in_smem = 0;
@@ -163,11 +168,11 @@ namespace {
 struct ProfScope {
   sim* s; int k; bool is_kernel; cudaEvent_t a = nullptr, b = nullptr;
   ProfScope(sim* s_, int k_, bool is_kernel_ = true) : s(s_), k(k_), is_kernel(is_kernel_) {
-    if (s->profile) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, s->stream); }
+    if (s->profile) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, s->run); }
   }
   ~ProfScope() {
     if (is_kernel) s->launches++;   // memsets are not kernels of ours
-    if (s->profile) { cudaEventRecord(b, s->stream); s->prof_pending.push_back({k, {a, b}}); }
+    if (s->profile) { cudaEventRecord(b, s->run); s->prof_pending.push_back({k, {a, b}}); }
   }
 };
 
@@ -210,27 +215,71 @@ int enqueue_step(sim* s) {
   Params& p = s->prm;
   {
     ProfScope ps(s, KI_CELL_ZERO, false);
-    CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->stream));
+    CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->run));
   }
   { ProfScope ps(s, KI_MOVE);
-    k_move_hist<<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(p, s->gauss_in_smem); }
+    k_move_hist<<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p, s->gauss_in_smem); }
   { ProfScope ps(s, KI_CELL_REDUCE);
-    k_cell_reduce<<<kScanBlocks, kScanThreads, 0, s->stream>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+    k_cell_reduce<<<kScanBlocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_CELL_SCAN);
-    k_cell_scan<<<kScanBlocks, kScanThreads, 0, s->stream>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+    k_cell_scan<<<kScanBlocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_SCATTER);
-    k_scatter<<<s->grid_scatter, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(p, s->gauss_in_smem); }
-  { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_BIRTH_REDUCE); k_birth_reduce<<<kBirthBlocks, kScanThreads, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_BIRTH_SCAN); k_birth_scan<<<kBirthBlocks, kScanThreads, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_BIRTHS); k_births<<<148, 128, 0, s->stream>>>(p); }
-  { ProfScope ps(s, KI_EPILOGUE); k_epilogue<<<148, 256, 0, s->stream>>>(p); }
+    k_scatter<<<s->grid_scatter, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p, s->gauss_in_smem); }
+  { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_BIRTH_REDUCE); k_birth_reduce<<<kBirthBlocks, kScanThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_BIRTH_SCAN); k_birth_scan<<<kBirthBlocks, kScanThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_BIRTHS); k_births<<<148, 128, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_EPILOGUE); k_epilogue<<<148, 256, 0, s->run>>>(p); }
   CK(cudaGetLastError());
   std::swap(p.cur, p.oth);   // the sorted copy (+ newborns) is the next step's current state
   s->t_host++;
   return SIM_OK;
+}
+
+}  // namespace
+
+namespace {
+
+constexpr uint32_t kGraphSteps = 8;   // even, so the parity after the graph equals the parity before
+
+int parity_of(const sim* s) { return s->prm.cur.x == (const int32_t*)(s->ws + s->lay.soa[0][0]) ? 0 : 1; }
+
+// Captures `steps` steps starting at the current parity into an executable graph; the handle's
+// host-side state is restored afterwards (capturing executes nothing).
+bool capture_steps(sim* s, uint32_t steps, cudaGraphExec_t* out) {
+  const Params saved = s->prm;
+  const uint64_t launches = s->launches;
+  const uint32_t t_host = s->t_host;
+  cudaGraph_t graph = nullptr;
+  bool ok = cudaStreamBeginCapture(s->cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (ok) {
+    s->run = s->cap;
+    for (uint32_t k = 0; k < steps && ok; ++k) ok = enqueue_step(s) == SIM_OK;
+    s->run = s->stream;
+    ok = (cudaStreamEndCapture(s->cap, &graph) == cudaSuccess) && ok && graph;
+  }
+  if (ok) ok = cudaGraphInstantiate(out, graph, 0) == cudaSuccess;
+  if (graph) cudaGraphDestroy(graph);
+  if (ok) s->kernels_per_step = (uint32_t)((s->launches - launches) / steps);
+  s->prm = saved; s->launches = launches; s->t_host = t_host;
+  if (!ok) cudaGetLastError();
+  return ok;
+}
+
+// The 12 launches of a step are replayed as CUDA graphs (one step, or 8 steps, per starting parity of
+// the cur/oth ping-pong): the path is launch-bound below ~1 M agents.
+void build_graphs(sim* s) {
+  s->graphs_tried = true;
+  if (cudaStreamCreateWithFlags(&s->cap, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return; }
+  bool ok = true;
+  for (int k = 0; k < 2 && ok; ++k) {
+    const int par = parity_of(s);
+    ok = capture_steps(s, 1, &s->g1[par]) && capture_steps(s, kGraphSteps, &s->g8[par]);
+    std::swap(s->prm.cur, s->prm.oth);   // the other parity (swapped back by the second round)
+  }
+  s->graphs_ok = ok;
 }
 
 }  // namespace
@@ -260,6 +309,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   s->lay = L;
   s->ws = (char*)d_workspace;
   s->stream = (cudaStream_t)cuda_stream;
+  s->run = s->stream;
 
   // host image of the device tables
   std::vector<DevTables> tabv(1);
@@ -381,6 +431,11 @@ void sim_destroy(sim_t* s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
   prof_collect(s);
+  for (int k = 0; k < 2; ++k) {
+    if (s->g1[k]) cudaGraphExecDestroy(s->g1[k]);
+    if (s->g8[k]) cudaGraphExecDestroy(s->g8[k]);
+  }
+  if (s->cap) cudaStreamDestroy(s->cap);
   delete s;
 }
 
@@ -418,7 +473,21 @@ int sim_step_async(sim_t* s, uint32_t n_steps) {
   if (!s) return SIM_E_INVAL;
   if (s->sticky) return s->sticky;
   if ((uint64_t)s->t_host + n_steps >= s->cfg.counts_rows) return SIM_E_CAPACITY;
-  for (uint32_t i = 0; i < n_steps; ++i) {
+  if (!s->profile && !s->graphs_tried) build_graphs(s);
+  uint32_t left = n_steps;
+  if (!s->profile && s->graphs_ok) {
+    while (left >= kGraphSteps) {
+      CK(cudaGraphLaunch(s->g8[parity_of(s)], s->stream));
+      s->t_host += kGraphSteps; s->launches += (uint64_t)s->kernels_per_step * kGraphSteps; left -= kGraphSteps;
+    }
+    while (left) {
+      CK(cudaGraphLaunch(s->g1[parity_of(s)], s->stream));
+      std::swap(s->prm.cur, s->prm.oth);
+      s->t_host++; s->launches += s->kernels_per_step; --left;
+    }
+    return SIM_OK;
+  }
+  for (uint32_t i = 0; i < left; ++i) {   // per-kernel profiling (events between launches), or no graph support
     int r = enqueue_step(s);
     if (r) return r;
   }
