@@ -16,10 +16,10 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
                                                uint32_t k0, uint32_t k1) {
 #pragma unroll
   for (int round = 0; round < 10; ++round) {
-    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-    const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;   // one IMAD.WIDE gives hi and lo
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c0 = n0; c1 = (uint32_t)p1; c2 = n2; c3 = (uint32_t)p0;
     k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;   // the bump after the last round is dead code
   }
   return make_uint4(c0, c1, c2, c3);
@@ -109,7 +109,8 @@ __device__ __forceinline__ Moved move_agent(const Params& p, const MoveTables& M
 
 // Gaussian inverse-CDF tables (north_star (2)) and the species / compartment fields are staged in
 // shared memory once per (persistent) block.
-__device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTables& M, int16_t* s_gauss, int gauss_in_smem) {
+template <bool kGaussSmem>
+__device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTables& M, int16_t* s_gauss) {
   const DevTables* __restrict__ T = p.tab;
   for (uint32_t k = threadIdx.x; k < (uint32_t)kMaxSpecies; k += blockDim.x) {
     const DevSpecies& S = T->sp[k];
@@ -117,7 +118,7 @@ __device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTabl
   }
   for (uint32_t k = threadIdx.x; k < (uint32_t)kMaxCompartments; k += blockDim.x) M.comp[k] = T->comp[k];
   const int16_t* g = p.gauss;
-  if (gauss_in_smem) {
+  if (kGaussSmem) {
     const uint32_t n_words = (p.n_classes << p.table_bits) >> 1;      // table_bits >= 1: an even number of int16
     const uint32_t* src = reinterpret_cast<const uint32_t*>(p.gauss);
     uint32_t* dst = reinterpret_cast<uint32_t*>(s_gauss);
@@ -142,10 +143,11 @@ __device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTabl
 constexpr int kMoveUnroll = MOLSIM_MOVE_UNROLL;
 constexpr int kMoveThreads = 256;
 
-__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(Params p, int gauss_in_smem) {
+template <bool kGaussSmem>
+__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
-  const int16_t* g = stage_tables(p, M, s_gauss, gauss_in_smem);
+  const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   const uint32_t lane = threadIdx.x & 31u;
   constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
@@ -189,10 +191,11 @@ __global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(
 }
 
 // Test hook (sim_debug_move_only): phase 1 in place on the current arrays.
-__global__ void __launch_bounds__(kMoveThreads) k_move_only(Params p, int gauss_in_smem) {
+template <bool kGaussSmem>
+__global__ void __launch_bounds__(kMoveThreads) k_move_only(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
-  const int16_t* g = stage_tables(p, M, s_gauss, gauss_in_smem);
+  const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const uint16_t s = p.cur.sp[i];
@@ -260,10 +263,11 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
 // slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
 // kMoveUnroll agents in flight per thread.  Membrane crossings change the species here; their
 // counts deltas go straight to counts row t+1 (rare events).
-__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_scatter(Params p, int gauss_in_smem) {
+template <bool kGaussSmem>
+__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_scatter(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
-  const int16_t* g = stage_tables(p, M, s_gauss, gauss_in_smem);
+  const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
   constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;

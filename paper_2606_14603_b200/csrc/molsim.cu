@@ -218,13 +218,15 @@ int enqueue_step(sim* s) {
     CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->run));
   }
   { ProfScope ps(s, KI_MOVE);
-    k_move_hist<<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p, s->gauss_in_smem); }
+    if (s->gauss_in_smem) k_move_hist<true><<<s->grid_move, kMoveThreads, s->gauss_bytes, s->run>>>(p);
+    else k_move_hist<false><<<s->grid_move, kMoveThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_CELL_REDUCE);
     k_cell_reduce<<<kScanBlocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_CELL_SCAN);
     k_cell_scan<<<kScanBlocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_SCATTER);
-    k_scatter<<<s->grid_scatter, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p, s->gauss_in_smem); }
+    if (s->gauss_in_smem) k_scatter<true><<<s->grid_scatter, kMoveThreads, s->gauss_bytes, s->run>>>(p);
+    else k_scatter<false><<<s->grid_scatter, kMoveThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
@@ -393,13 +395,15 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     int occ = 0;
     const size_t gsm = s->gauss_in_smem ? s->gauss_bytes : 0;
     if (gsm > 48 * 1024) {
-      cudaFuncSetAttribute(k_move_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
-      cudaFuncSetAttribute(k_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
-      cudaFuncSetAttribute(k_move_only, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(k_move_hist<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(k_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(k_move_only<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
     }
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hist, kMoveThreads, gsm);
+    if (gsm) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hist<true>, kMoveThreads, gsm);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hist<false>, kMoveThreads, 0);
     s->grid_move = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter, kMoveThreads, gsm);
+    if (gsm) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter<true>, kMoveThreads, gsm);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter<false>, kMoveThreads, 0);
     s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
     s->grid_pairs = (uint32_t)(((uint64_t)cfg->capacity + kPairThreads - 1) / kPairThreads);   // one tile per block
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, kUniThreads, 0);
@@ -601,7 +605,8 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
 int sim_debug_move_only(sim_t* s) {
   if (!s) return SIM_E_INVAL;
   { ProfScope ps(s, KI_MOVE);
-    k_move_only<<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(s->prm, s->gauss_in_smem); }
+    if (s->gauss_in_smem) k_move_only<true><<<s->grid_move, kMoveThreads, s->gauss_bytes, s->stream>>>(s->prm);
+    else k_move_only<false><<<s->grid_move, kMoveThreads, 0, s->stream>>>(s->prm); }
   CK(cudaGetLastError());
   // crossing deltas went to row t+1: fold them back so that row t describes the moved state
   Scalars sc;
