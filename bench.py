@@ -127,9 +127,10 @@ def ledger_bytes_per_agent(kernel, c):
 
 def moved_bytes_per_agent(kernel, c):
     """What THIS implementation must move per live agent per launch: smaller than the
-    §8(d) ledger where a pass was elided (sparse proposals), larger where it keeps an extra array (off)."""
+    §8(d) ledger where a pass was elided (move recomputed in K3, sparse proposals), larger where it keeps an
+    extra array (off)."""
     return {
-        "k_move_hist": 18 + 12 + 4 + 8 * c,      # R soa, W xyz, W off, cell count RMW
+        "k_move_hist": 18 + 4 + 8 * c,           # R soa, W off, cell count RMW (moved positions are not stored)
         "memset_cells": 4 * c, "k_cell_reduce": 4 * c, "k_cell_scan": 8 * c,
         "k_scatter": 18 + 4 + 18 + 4 * c,        # R soa + off, W soa, R cell starts
         "k_pairs": 14 + 0.125 + 4 * c,           # R xyz + species, W 1 bit; R cell starts
@@ -371,7 +372,7 @@ def main():
     ap.add_argument("--cell-size", type=int, default=0)
     ap.add_argument("--prof-steps", type=int, default=5)
     ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--cpu-n", type=int, default=16_000_000, help="oracle sample size for cpu_baseline")
+    ap.add_argument("--cpu-n", type=int, default=4_000_000, help="oracle sample size for cpu_baseline")
     ap.add_argument("--cpu-steps", type=int, default=1)
     ap.add_argument("--ref-n", type=int, default=1_000_000, help="oracle sample size for --impl reference")
     ap.add_argument("--no-cpu", action="store_true")
