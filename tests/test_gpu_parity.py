@@ -223,6 +223,25 @@ def test_w4_16m_full_size_two_steps(gpu):
     run_both(gpu, m, 2, chunks=1)
 
 
+def test_w1_full_size_steps(gpu):
+    """[CFG 1] at full size (1.05 M agents, sphere R = 5 um) in the bench launch configuration."""
+    m = configs.w1(n_steps=4)
+    run_both(gpu, m, 4, chunks=2)
+
+
+def test_w3_full_size_steps(gpu):
+    """[CFG 3] at full size (337,502 agents, shell + nucleus, membrane crossings)."""
+    m = configs.w3(n_steps=24)
+    run_both(gpu, m, 24, chunks=2)
+
+
+@pytest.mark.slow
+def test_w2_full_size_two_steps(gpu):
+    """[CFG 2] at full size: 8 replicas, 8,854,860 agents, every agent compared with the oracle."""
+    m = configs.w2(n_steps=2)
+    run_both(gpu, m, 2, chunks=1)
+
+
 def test_errors(gpu):
     from paper_2606_14603_b200.binding import E_CAPACITY, E_INVAL, SimError
 
