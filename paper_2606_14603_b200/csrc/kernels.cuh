@@ -346,8 +346,8 @@ __device__ __forceinline__ void delta_flush(const int32_t* s_delta, uint32_t* __
 //     need, are pushed as 16-bit tasks (owner, row code) into the warp's shared list and
 //  C  scanned by the whole warp, 1, 2 or 4 lanes per task, so the few lanes that need them do not
 //     stall the others.
-//  D  geometric hits (dist^2 <= R^2: a fraction of a percent of the candidates) were only queued;
-//     now one lane per hit does the reaction lookup and the pair draw and, if the pair qualifies,
+//  D  window hits (|d| <= R on every axis: a fraction of a percent of the candidates) were only queued;
+//     now one lane per hit does the exact distance, the reaction lookup and the pair draw and, if the pair qualifies,
 //     the two atomicMin.  best[] is touched only there (rare), so it costs no bandwidth; hasprop
 //     gets one bit per touched agent and bslot[] the slot of the partner that lowered the key.
 //     Two lanes lowering the same key may store their slots in either order, so K4b checks
@@ -378,7 +378,7 @@ __device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t
 constexpr int kWarpTaskCap = 128;       // 4 forward rows x 32 agents: always fits
 constexpr int kWarpHitCap = 64;
 struct PairWarpSmem {                   // private to one warp
-  uint32_t hit_j[kWarpHitCap], hit_d[kWarpHitCap];
+  uint32_t hit_j[kWarpHitCap];          // candidate slot that passed the window test
   uint8_t hit_o[kWarpHitCap];           // owner thread
   uint16_t task[kWarpTaskCap];          // owner thread | row code (5..8) << 8
   uint32_t nhit;
@@ -389,9 +389,9 @@ struct PairSmem {
   PairWarpSmem w[kPairThreads / 32];
 };
 
-__device__ __forceinline__ void push_hit(PairWarpSmem& W, uint32_t owner, uint32_t j, uint32_t d2) {
+__device__ __forceinline__ void push_hit(PairWarpSmem& W, uint32_t owner, uint32_t j) {
   const uint32_t h = atomicAdd(&W.nhit, 1u);
-  if (h < (uint32_t)kWarpHitCap) { W.hit_j[h] = j; W.hit_d[h] = d2; W.hit_o[h] = (uint8_t)owner; }
+  if (h < (uint32_t)kWarpHitCap) { W.hit_j[h] = j; W.hit_o[h] = (uint8_t)owner; }
 }
 
 // Tile slots [ka, kb) (shared memory) against the agent `owner` at (x, y, z).
@@ -404,11 +404,7 @@ __device__ __forceinline__ void scan_tile(const Params& p, const PairSmem& S, Pa
   for (uint32_t k = ka; k < kb; ++k) {
     const int4 q = S.pos[k];
     const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
-    if (max(max(ux, uy), uz) <= R2) {
-      const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
-      const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (d2 <= p.max_r2) push_hit(W, owner, base + k, d2);
-    }
+    if (max(max(ux, uy), uz) <= R2) push_hit(W, owner, base + k);   // |d| <= R on every axis: D looks closer
   }
 }
 
@@ -424,11 +420,7 @@ __device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, ui
 #pragma unroll 2
   for (uint32_t j = j0; j < j1; ++j) {
     const uint32_t ux = (uint32_t)(__ldg(X + j) + ox), uy = (uint32_t)(__ldg(Y + j) + oy), uz = (uint32_t)(__ldg(Z + j) + oz);
-    if (max(max(ux, uy), uz) <= R2) {
-      const int32_t dx = (int32_t)ux - R, dy = (int32_t)uy - R, dz = (int32_t)uz - R;
-      const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (d2 <= p.max_r2) push_hit(W, owner, j, d2);
-    }
+    if (max(max(ux, uy), uz) <= R2) push_hit(W, owner, j);
   }
 }
 
@@ -494,22 +486,13 @@ __global__ void __launch_bounds__(kPairThreads, 6) k_pairs(const __grid_constant
     if (j1 > base + kPairThreads) scan_global(p, W, base + kPairThreads, j1, tid, x, y, z);
   }
 
-  // ---- B: the warp's task list (exclusive scan of the task counts)
-  const uint32_t my_tasks = __popc(need);
-  uint32_t incl = my_tasks;
+  // ---- B: the warp's task list: one ballot per forward row code
+  uint32_t nt = 0;
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-    if (lane >= (uint32_t)d) incl += o;
-  }
-  const uint32_t nt = __shfl_sync(0xFFFFFFFFu, incl, 31);
-  {
-    uint32_t pos = incl - my_tasks, m = need;
-    while (m) {
-      const uint32_t c = __ffs(m) - 1u;
-      m &= m - 1u;
-      W.task[pos++] = (uint16_t)(tid | (c << 8));
-    }
+  for (uint32_t c = 5u; c <= 8u; ++c) {
+    const uint32_t m = __ballot_sync(0xFFFFFFFFu, (need >> c) & 1u);
+    if ((need >> c) & 1u) W.task[nt + __popc(m & ((1u << lane) - 1u))] = (uint16_t)(tid | (c << 8));
+    nt += __popc(m);
   }
   __syncwarp();
 
@@ -527,12 +510,15 @@ __global__ void __launch_bounds__(kPairThreads, 6) k_pairs(const __grid_constant
   }
   __syncwarp();
 
-  // ---- D: qualify the queued hits, one lane per hit
+  // ---- D: qualify the queued hits, one lane per hit: exact distance, then reaction look-up and draw
   const uint32_t nh = W.nhit;
   if (nh <= (uint32_t)kWarpHitCap) {
     for (uint32_t h = lane; h < nh; h += 32u) {
-      const uint32_t owner = W.hit_o[h];
-      pair_merge(p, base + owner, W.hit_j[h], W.hit_d[h], (uint32_t)S.pos[owner].w, t);
+      const uint32_t owner = W.hit_o[h], j = W.hit_j[h];
+      const int4 q = S.pos[owner];
+      const int32_t dx = p.oth.x[j] - q.x, dy = p.oth.y[j] - q.y, dz = p.oth.z[j] - q.z;   // each within +-R
+      const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
+      if (d2 <= p.max_r2) pair_merge(p, base + owner, j, d2, (uint32_t)q.w, t);
     }
   } else if (active) {
     slow_agent(&p, i, x, y, z, s, rowc, xlo, nxr, j1, need, t);
