@@ -55,7 +55,7 @@ def w0(cell_size: int = 50, n_steps: int = 1000, seed: int = 1) -> Model:
 W4_EDGES = {1_000_000: 32_183, 4_000_000: 51_087, 16_000_000: 81_096, 64_000_000: 128_732}
 
 
-def w4(n: int = 16_000_000, cell_size: int = 512, n_steps: int = 100) -> Model:
+def w4(n: int = 16_000_000, cell_size: int = 448, n_steps: int = 100) -> Model:
     """[CFG 4]: fixed density 30,000 agents/um^3 (reading S21 for the cube edges)."""
     if n in W4_EDGES:
         L = W4_EDGES[n]
