@@ -384,8 +384,8 @@ struct PairWarpSmem {                   // private to one warp
   uint32_t nhit;
 };
 struct PairSmem {
-  int4 pos[kPairThreads];               // x, y, z, species
-  uint32_t row[kPairThreads], xr[kPairThreads];
+  int4 pos[kPairThreads];               // x, y, z, species | forward-row mask << 16
+  uint32_t row[kPairThreads], xr[kPairThreads];   // own row's first cell; first x cell | (x cells - 1) << 30
   PairWarpSmem w[kPairThreads / 32];
 };
 
@@ -432,16 +432,21 @@ __device__ __forceinline__ uint32_t row_of(const Params& p, uint32_t rowc, uint3
 }
 
 // Plain per-thread forward search with immediate merge: used by warps whose hit queue overflowed.
-__device__ __noinline__ void slow_agent(const Params* pp, uint32_t i, int32_t x, int32_t y, int32_t z, uint32_t si,
-                                        uint32_t rowc, uint32_t xlo, uint32_t nxr, uint32_t j1_own, uint32_t need, uint32_t t) {
+// Everything it needs is read back from the tile in shared memory, so the fast path keeps no
+// registers alive for it.
+__device__ __noinline__ void slow_agent(const Params* pp, const PairSmem* Sp, uint32_t tid, uint32_t i, uint32_t t) {
   const Params& p = *pp;
+  const int4 q = Sp->pos[tid];
+  const int32_t x = q.x, y = q.y, z = q.z;
+  const uint32_t si = (uint32_t)q.w & 0xFFFFu, rowc = Sp->row[tid], xr = Sp->xr[tid];
+  const uint32_t xlo = xr & 0x3FFFFFFFu, nxr = xr >> 30;
+  uint32_t need = ((uint32_t)q.w >> 16) | (1u << 4);
   const long long R = p.max_r;
-  need |= 1u << 4;
   while (need) {
     const uint32_t c = __ffs(need) - 1u;
     need &= need - 1u;
     const uint32_t r2 = row_of(p, rowc, c);
-    const uint32_t j0 = c == 4u ? i + 1u : p.cell[r2 + xlo], j1 = c == 4u ? j1_own : p.cell[r2 + xlo + nxr + 1];
+    const uint32_t j0 = c == 4u ? i + 1u : p.cell[r2 + xlo], j1 = p.cell[r2 + xlo + nxr + 1];
     for (uint32_t j = j0; j < j1; ++j) {
       const long long dx = (long long)p.oth.x[j] - x, dy = (long long)p.oth.y[j] - y, dz = (long long)p.oth.z[j] - z;
       if (dx > R || dx < -R || dy > R || dy < -R || dz > R || dz < -R) continue;
@@ -482,7 +487,7 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
     need = (yp << 5) | (zp ? ((ym | 2u | (yp << 2)) << 6) : 0u);
     j1 = p.cell[rowc + (uint32_t)cx + xp + 1u];            // end of the own-row forward range, > i
   }
-  S.pos[tid] = make_int4(x, y, z, (int32_t)s);
+  S.pos[tid] = make_int4(x, y, z, (int32_t)(s | (need << 16)));    // species | forward-row mask << 16
   S.row[tid] = rowc; S.xr[tid] = xlo | (nxr << 30);
   __syncthreads();          // the only block-wide barrier: the tile is read-only from here on
 
@@ -524,10 +529,10 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
       const int4 q = S.pos[owner];
       const int32_t dx = p.oth.x[j] - q.x, dy = p.oth.y[j] - q.y, dz = p.oth.z[j] - q.z;   // each within +-R
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (d2 <= p.max_r2) pair_merge(p, base + owner, j, d2, (uint32_t)q.w, t);
+      if (d2 <= p.max_r2) pair_merge(p, base + owner, j, d2, (uint32_t)q.w & 0xFFFFu, t);
     }
   } else if (active) {
-    slow_agent(&p, i, x, y, z, s, rowc, xlo, nxr, j1, need, t);
+    slow_agent(&p, &S, tid, i, t);
   }
 }
 
