@@ -76,6 +76,7 @@ struct Params {
   const DevTables* tab;
   const int16_t* gauss;     // [n_classes << B]
   uint32_t key0, key1;
+  uint32_t rk0[10], rk1[10];   // Philox round keys of the simulation key: key + round * bump
   uint32_t capacity, id_capacity;
   uint32_t n_species, n_replicas, stride_shift, table_bits, n_classes;
   int32_t cell_size;

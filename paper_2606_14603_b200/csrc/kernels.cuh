@@ -25,6 +25,20 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
   return make_uint4(c0, c1, c2, c3);
 }
 
+// The simulation streams all use the key (seed lo, seed hi): their ten round keys are precomputed on
+// the host into the kernel parameters, so a round is two IMAD.WIDE and two three-input XORs whose
+// key operand comes straight from the constant bank.
+__device__ __forceinline__ uint4 philox_sim(const Params& p, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
+#pragma unroll
+  for (int round = 0; round < 10; ++round) {
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ p.rk0[round], n2 = (uint32_t)(p0 >> 32) ^ c3 ^ p.rk1[round];
+    c0 = n0; c1 = (uint32_t)p1; c2 = n2; c3 = (uint32_t)p0;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
 __global__ void k_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, uint32_t n) {
   uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -91,7 +105,7 @@ __device__ __forceinline__ Moved move_agent(const Params& p, const MoveTables& M
   const uint32_t cls = S.cls;
   if (!cls) return m;
   const uint32_t sh = 32u - p.table_bits;
-  const uint4 r = philox4x32_10(id, 0u, t, kTagMove, p.key0, p.key1);
+  const uint4 r = philox_sim(p, id, 0u, t, kTagMove);
   const int16_t* tb = g + (cls << p.table_bits);
   const int32_t rbase = (int32_t)(((uint32_t)x >> p.stride_shift) << p.stride_shift);
   int32_t qx = x - rbase + tb[r.x >> sh], qy = y + tb[r.y >> sh], qz = z + tb[r.z >> sh];
@@ -366,7 +380,7 @@ __device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t
   const DevRx& rx = T->rx[e];
   if (d2 > rx.r2) return;
   const uint32_t id = p.oth.id[i], idj = p.oth.id[j];
-  const uint4 r = philox4x32_10(min(id, idj), max(id, idj), t, kTagPair, p.key0, p.key1);
+  const uint4 r = philox_sim(p, min(id, idj), max(id, idj), t, kTagPair);
   if (!fire(r.x, rx.thr)) return;
   const unsigned long long hi = (unsigned long long)d2 << 32, ki = hi | idj, kj = hi | id;
   if (atomicMin(&p.best[i], ki) > ki) p.prop[i] = j;
@@ -601,7 +615,7 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
   const DevSpecies& S = T->sp[s0];
   const uint32_t nch = S.n_channels;
   const uint32_t id = p.oth.id[i];
-  const uint4 r = philox4x32_10(id, 0u, t, kTagUni, p.key0, p.key1);
+  const uint4 r = philox_sim(p, id, 0u, t, kTagUni);
   const uint32_t rr[4] = {r.x, r.y, r.z, r.w};
   bool consumed = false;
   uint16_t s = s0;
@@ -786,7 +800,7 @@ __global__ void __launch_bounds__(128) k_births(Params p) {
     for (uint32_t k = 0; k < 4u; ++k) {
       if (!(mask >> k & 1u)) continue;
       const uint16_t sp_new = T->sp[pre].ch[k].prod1;
-      const uint4 r = philox4x32_10(pid, k, t, kTagBirth, p.key0, p.key1);
+      const uint4 r = philox_sim(p, pid, k, t, kTagBirth);
       int32_t qx = lx + (int32_t)__umulhi(r.x, 21u) - 10;
       int32_t qy = py + (int32_t)__umulhi(r.y, 21u) - 10;
       int32_t qz = pz + (int32_t)__umulhi(r.z, 21u) - 10;

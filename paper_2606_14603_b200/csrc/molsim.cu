@@ -361,6 +361,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   p.birth_list = (uint2*)(w + L.birth_list); p.counts = (uint32_t*)(w + L.counts);
   p.scal = (Scalars*)(w + L.scal); p.tab = (const DevTables*)(w + L.tab); p.gauss = (const int16_t*)(w + L.gauss);
   p.key0 = (uint32_t)cfg->seed; p.key1 = (uint32_t)(cfg->seed >> 32);
+  for (uint32_t r = 0; r < 10; ++r) { p.rk0[r] = p.key0 + r * 0x9E3779B9u; p.rk1[r] = p.key1 + r * 0xBB67AE85u; }
   p.capacity = cfg->capacity; p.id_capacity = cfg->id_capacity;
   p.n_species = cfg->n_species; p.n_replicas = cfg->n_replicas; p.stride_shift = cfg->stride_shift;
   p.table_bits = cfg->table_bits; p.n_classes = cfg->n_sigma_classes;
