@@ -202,6 +202,19 @@ def cpu_baseline(args):
             "host_cpus": os.cpu_count()}
 
 
+def reduce_ranks(times, work, device):
+    """N independent replicas: the job's time is the MAX over ranks, its work the SUM.
+    Uses whatever process group is initialised (nccl on the GPU box, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+
+    tt = torch.tensor(list(times), dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ww = torch.tensor(list(work), dtype=torch.float64, device=device)
+    dist.all_reduce(ww, op=dist.ReduceOp.SUM)
+    return tt.tolist(), ww.tolist()
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -317,12 +330,8 @@ def run_gpu(args):
 
     # ---- reduce over ranks: max time, summed work
     if world > 1:
-        tt = torch.tensor([ms, e2e_dt], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ww = torch.tensor([agent_steps, e2e_agent_steps, float(launches)], dtype=torch.float64, device=dev)
-        dist.all_reduce(ww, op=dist.ReduceOp.SUM)
-        ms, e2e_dt = tt.tolist()
-        agent_steps, e2e_agent_steps, launches = ww.tolist()
+        (ms, e2e_dt), (agent_steps, e2e_agent_steps, launches) = reduce_ranks(
+            [ms, e2e_dt], [agent_steps, e2e_agent_steps, float(launches)], dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

@@ -114,7 +114,7 @@ def test_tiny_dense_cube_many_events(gpu):
 def test_cell_size_independence_on_gpu(gpu):
     m = tiny_cube(L=400, n_a=1500, n_b=1500, p_rel=0.02)
     ref = None
-    for cell in (50, 64, 100, 256, 400):
+    for cell in (50, 53, 64, 97, 100, 256, 333, 400):   # odd sizes exercise the multiply-high cell division
         sim = gpu.Sim(m, cell_size=cell); sim.seed_population(); sim.step(12)
         s = sim.read_agents()
         if ref is None:
