@@ -126,7 +126,9 @@ int sim_read_agents(sim_t*, uint32_t cap, int32_t* x, int32_t* y, int32_t* z,
                     uint16_t* species, uint32_t* id, uint32_t* n_out);
 
 /* Replaces the population by explicit agents in any order (checkpoint reload / test hook);
- * sets the step counter and next_id; rewrites counts row `step`.  HOST arrays. */
+ * sets the step counter and next_id; rewrites counts row `step`.  HOST arrays (pinned memory makes
+ * the copies asynchronous).  Species, replica tile (x >> stride_shift) and id < next_id of every
+ * agent are validated on the device: on SIM_E_INVAL the handle holds an EMPTY population. */
 int sim_load_agents(sim_t*, uint32_t n, const int32_t* x, const int32_t* y, const int32_t* z,
                     const uint16_t* species, const uint32_t* id, uint32_t step, uint32_t next_id);
 

@@ -588,7 +588,7 @@ __global__ void __launch_bounds__(256) k_resolve(const __grid_constant__ Params 
       const uint32_t idj = (uint32_t)p.best[i];            // low word of (d2, id of the proposed partner)
       uint32_t j = p.prop[i];
       if (j >= n || p.oth.id[j] != idj) j = find_partner(&p, i, idj);
-      if (j <= i) continue;                                   // the lower slot handles the pair
+      if (j <= i || j >= n) continue;                         // the lower slot handles the pair
       const uint32_t idi = p.oth.id[i];
       if ((uint32_t)p.best[j] != idi) continue;               // not mutual (best[j] = kNoKey if j never proposed)
       const uint16_t si = p.oth.sp[i], sj = p.oth.sp[j];
@@ -881,10 +881,14 @@ __global__ void k_seed(Params p, uint32_t species, uint32_t replica, uint32_t co
 __global__ void __launch_bounds__(256) k_count_row(Params p, uint32_t r, uint32_t n_slots) {
   __shared__ int32_t s_delta[kMaxRowWidth];
   delta_zero(s_delta, p.row_width);
+  const uint32_t next_id = p.scal->next_id;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += gridDim.x * blockDim.x) {
     const uint16_t s = p.cur.sp[i];
     if (s == kDead) continue;
-    atomicAdd(&s_delta[((uint32_t)p.cur.x[i] >> p.stride_shift) * p.n_species + s], 1);
+    const uint32_t rep = (uint32_t)p.cur.x[i] >> p.stride_shift;
+    // sim_load_agents hands us caller data: species, replica tile and id are validated here (err bit 2)
+    if (s >= p.n_species || rep >= p.n_replicas || p.cur.id[i] >= next_id) { atomicOr(&p.scal->err, 4u); continue; }
+    atomicAdd(&s_delta[rep * p.n_species + s], 1);
   }
   delta_flush(s_delta, p.counts + (size_t)r * p.row_width, p.row_width);
 }

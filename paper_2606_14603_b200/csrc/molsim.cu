@@ -194,6 +194,7 @@ int read_scalars(sim* s, Scalars* out) {
 }
 
 int err_from_bits(uint32_t bits) {
+  if (bits & 4u) return SIM_E_INVAL;
   if (bits & 1u) return SIM_E_CAPACITY;
   if (bits & 2u) return SIM_E_IDSPACE;
   return SIM_OK;
@@ -584,7 +585,6 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
   if (!s || n > s->cfg.capacity || (uint64_t)step + 1 > s->cfg.counts_rows || next_id > s->cfg.id_capacity)
     return SIM_E_INVAL;
   if (n && (!x || !y || !z || !species || !id)) return SIM_E_INVAL;
-  for (uint32_t i = 0; i < n; ++i) if (species[i] >= s->cfg.n_species || id[i] >= next_id) return SIM_E_INVAL;
   Scalars sc;
   int r = read_scalars(s, &sc);
   if (r) return r;
@@ -597,9 +597,19 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
   sc.birth_count = sc.total_births = sc.ticket = 0;
   CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
   s->t_host = step; s->sticky = SIM_OK;
-  r = recount_row(s, step, n);
+  r = recount_row(s, step, n);   // also validates species / replica tile / id of every agent on the device
   if (r) return r;
+  uint32_t err = 0;
+  CK(cudaMemcpyAsync(&err, &s->prm.scal->err, 4, cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
+  if (err & 4u) {                 // invalid agent data: leave an empty, usable population behind
+    sc.n_slots = 0; sc.err = 0;
+    CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
+    r = recount_row(s, step, 0);
+    if (r) return r;
+    CK(cudaStreamSynchronize(s->stream));
+    return SIM_E_INVAL;
+  }
   return SIM_OK;
 }
 

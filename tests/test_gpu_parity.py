@@ -259,6 +259,21 @@ def test_errors(gpu):
     with pytest.raises(SimError) as e:      # every C releases a newborn: 4,000 > capacity
         sim.step(1)
     assert e.value.code == E_CAPACITY
+    # agent data handed to sim_load_agents is validated on the device; the handle stays usable
+    m = tiny_cube()
+    sim = gpu.Sim(m)
+    ok = np.arange(10, dtype=np.uint32)
+    xs = np.full(10, 5, np.int32)
+    for bad in ({"species": np.full(10, 7, np.uint16)}, {"id": ok + 100}, {"x": np.full(10, -3, np.int32)}):
+        a = {"x": xs, "y": xs, "z": xs, "species": np.zeros(10, np.uint16), "id": ok}
+        a.update(bad)
+        with pytest.raises(SimError) as e:
+            sim.load_agents(a["x"], a["y"], a["z"], a["species"], a["id"], next_id=10)
+        assert e.value.code == E_INVAL
+        assert sim.info()["n_live"] == 0
+    sim.load_agents(xs, xs, xs, np.zeros(10, np.uint16), ok, next_id=10)
+    sim.step(2)
+    assert sim.info()["n_live"] == 10
     m = tiny_cube(); m.counts_rows = 4
     sim = gpu.Sim(m); sim.seed_population(); sim.step(3)
     with pytest.raises(SimError):
