@@ -92,10 +92,11 @@ struct Params {
 
 __device__ __forceinline__ bool fire(uint32_t u, uint32_t thr) { return thr == 0xFFFFFFFFu || u < thr; }
 
+// Mirror about -1/2 and L - 1/2 (S5), branch-free: -1 - q == ~q, and for 0 <= a < 2L the reflected
+// value 2L - 1 - a is the smaller of the two exactly when a >= L (one reflection suffices: validated).
 __device__ __forceinline__ int32_t mirror(int32_t q, int32_t L) {
-  if (q < 0) return -1 - q;
-  if (q >= L) return 2 * L - 1 - q;
-  return q;
+  const int32_t a = q ^ (q >> 31);
+  return min(a, 2 * L - 1 - a);
 }
 
 __device__ __forceinline__ bool comp_valid(const DevComp& c, int32_t x, int32_t y, int32_t z) {
