@@ -111,6 +111,19 @@ def test_tiny_dense_cube_many_events(gpu):
     run_both(gpu, m, 40, chunks=8)
 
 
+def test_large_displacements(gpu):
+    # sigma = 300 / 250 units: displacements up to +-1100, several cells per step (cell 100)
+    A, B, Cx = 0, 1, 2
+    m = Model(
+        name="bigsigma", species=[Species("A", 1), Species("B", 1),
+                                  Species("C", 2, channels=[Channel(CH_RELEASE, prob_to_thr(0.02), A, B)])],
+        reactions=[Reaction(A, B, Cx, 2500, prob_to_thr(0.5))],
+        compartments=[Compartment(SHAPE_CUBE, L=3000)], table_bits=12, tables=stack_tables([300.0, 250.0], 12),
+        extent=(3000,) * 3, seed=21, place_seed=22,
+        seed_records=[SeedRecord(A, 4000), SeedRecord(B, 4000)], n_steps=24, cell_size=100).finalize()
+    run_both(gpu, m, 24, chunks=3)
+
+
 def test_cell_size_independence_on_gpu(gpu):
     m = tiny_cube(L=400, n_a=1500, n_b=1500, p_rel=0.02)
     ref = None
