@@ -281,13 +281,23 @@ def run_gpu(args):
     n_live_prof = float(sim.read_counts(W + K, args.prof_steps).sum()) / args.prof_steps
     dom_bytes = ledger_bytes_per_agent(dom, n_cells / n_live_prof) * n_live_prof
     achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = None
+    traffic, alu = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(f"{args.workload}:{args.n}", {}).get(dom)
+            tj = json.load(open(tpath))
+            traffic = tj.get(f"{args.workload}:{args.n}", {}).get(dom)
+            ipa = tj.get("warp_instr_per_agent", {}).get(f"{args.workload}:{args.n}", {}).get(dom)
+            if ipa:
+                # issue roofline of the dominant kernel: warp-instructions per launch (ncu count per
+                # agent x live agents) / launch time, against SMs x 4 schedulers x 1 instruction per clock x SM clock
+                peak_ginstr = 148 * 4 * 1.965
+                ach = ipa * n_live_prof / (dom_ms * 1e-3) / 1e9
+                alu = {"bound": "alu", "achieved": ach, "peak": peak_ginstr, "unit": "G warp-instr/s",
+                       "frac": ach / peak_ginstr, "warp_instr_per_agent": ipa,
+                       "peak_source": "148 SMs x 4 warp schedulers x 1 instr/clk x 1.965 GHz (B200_PROFILING.md clocks)"}
         except Exception:
-            traffic = None
+            traffic, alu = None, None
     step_bytes = sum(ledger_bytes_per_agent(k, c_per_agent) for k in step_kernels) * n_live_mean
     moved_bytes = sum(moved_bytes_per_agent(k, c_per_agent) for k in step_kernels) * n_live_mean
     per_kernel = {k: {"ms": round(v[0] / v[1], 4), "share": round(v[0] / tot_ms, 4),
@@ -355,7 +365,7 @@ def run_gpu(args):
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                     "kernel_ms": dom_ms, "kernel_share_of_step": step_kernels[dom][0] / tot_ms,
+                     "kernel_ms": dom_ms, "kernel_share_of_step": step_kernels[dom][0] / tot_ms, "alu": alu,
                      "whole_step": {"achieved": step_bytes / (ms / K * 1e-3) / 1e9,
                                     "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
                                     "frac_of_8TBs_nominal": step_bytes / (ms / K * 1e-3) / 1e9 / 8000.0,
