@@ -15,8 +15,9 @@ using namespace molsim;
 
 namespace {
 
-constexpr int kScanBlocks = 592;          // 148 SMs x 4
-constexpr uint32_t kBirthBlocks = 296;    // 148 SMs x 2
+constexpr uint32_t kMaxScanBlocks = 592;  // 148 SMs x 4; small problems get proportionally smaller grids (launch-bound)
+constexpr uint32_t kMaxBirthBlocks = 296; // 148 SMs x 2
+constexpr uint32_t kMaxTailBlocks = 148;
 
 enum KernelId { KI_MOVE = 0, KI_CELL_ZERO, KI_CELL_REDUCE, KI_CELL_SCAN, KI_SCATTER, KI_PAIRS,
                 KI_RESOLVE, KI_UNI, KI_BIRTH_REDUCE, KI_BIRTH_SCAN, KI_BIRTHS, KI_EPILOGUE, KI_OTHER };
@@ -147,7 +148,7 @@ struct sim {
   int gauss_in_smem = 0;
   size_t gauss_bytes = 0;
   uint32_t grid_move = 0, grid_scatter = 0, grid_pairs = 0, grid_uni = 0, grid_resolve = 0;
-  uint32_t cell_seg = 0;
+  uint32_t cell_seg = 0, scan_blocks = 1, birth_blocks = 1, tail_blocks = 1;
   bool profile = false;
   float prof_ms[SIM_N_KERNELS] = {};
   uint32_t prof_n[SIM_N_KERNELS] = {};
@@ -222,19 +223,19 @@ int enqueue_step(sim* s) {
     if (s->gauss_in_smem) k_move_hist<true><<<s->grid_move, kMoveThreads, s->gauss_bytes, s->run>>>(p);
     else k_move_hist<false><<<s->grid_move, kMoveThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_CELL_REDUCE);
-    k_cell_reduce<<<kScanBlocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+    k_cell_reduce<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_CELL_SCAN);
-    k_cell_scan<<<kScanBlocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+    k_cell_scan<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_SCATTER);
     if (s->gauss_in_smem) k_scatter<true><<<s->grid_scatter, kMoveThreads, s->gauss_bytes, s->run>>>(p);
     else k_scatter<false><<<s->grid_scatter, kMoveThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_BIRTH_REDUCE); k_birth_reduce<<<kBirthBlocks, kScanThreads, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_BIRTH_SCAN); k_birth_scan<<<kBirthBlocks, kScanThreads, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_BIRTHS); k_births<<<148, 128, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_EPILOGUE); k_epilogue<<<148, 256, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_BIRTH_REDUCE); k_birth_reduce<<<s->birth_blocks, kScanThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_BIRTH_SCAN); k_birth_scan<<<s->birth_blocks, kScanThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_BIRTHS); k_births<<<s->tail_blocks, 128, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_EPILOGUE); k_epilogue<<<s->tail_blocks, 256, 0, s->run>>>(p); }
   CK(cudaGetLastError());
   std::swap(p.cur, p.oth);   // the sorted copy (+ newborns) is the next step's current state
   s->t_host++;
@@ -414,7 +415,11 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     s->grid_resolve = sized(occ, 256 * 32);
     if (cudaGetLastError() != cudaSuccess) { delete s; return SIM_E_CUDA; }
   }
-  s->cell_seg = (uint32_t)align_up(((size_t)L.n_cells + kScanBlocks - 1) / kScanBlocks, 1024);
+  auto clampu = [](uint64_t v, uint64_t lo, uint64_t hi) { return (uint32_t)std::min(std::max(v, lo), hi); };
+  s->scan_blocks = clampu(((uint64_t)L.n_cells + 4095) / 4096, 1, kMaxScanBlocks);          // >= 4 K cells per block
+  s->cell_seg = (uint32_t)align_up(((size_t)L.n_cells + s->scan_blocks - 1) / s->scan_blocks, 1024);
+  s->birth_blocks = clampu(((uint64_t)cfg->id_capacity / 64 + 4095) / 4096, 1, kMaxBirthBlocks);  // >= 4 K id chunks per block
+  s->tail_blocks = clampu(((uint64_t)cfg->capacity + 65535) / 65536, 2, kMaxTailBlocks);
 
   Scalars sc;
   std::memset(&sc, 0, sizeof(sc));
