@@ -134,9 +134,13 @@ __device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTabl
   const int16_t* g = p.gauss;
   if (kGaussSmem) {
     const uint32_t n_words = (p.n_classes << p.table_bits) >> 1;      // table_bits >= 1: an even number of int16
+    const uint32_t n_quads = n_words >> 2;                            // 128-bit copies, then the tail
+    const uint4* src4 = reinterpret_cast<const uint4*>(p.gauss);
+    uint4* dst4 = reinterpret_cast<uint4*>(s_gauss);
+    for (uint32_t k = threadIdx.x; k < n_quads; k += blockDim.x) dst4[k] = src4[k];
     const uint32_t* src = reinterpret_cast<const uint32_t*>(p.gauss);
     uint32_t* dst = reinterpret_cast<uint32_t*>(s_gauss);
-    for (uint32_t k = threadIdx.x; k < n_words; k += blockDim.x) dst[k] = src[k];
+    for (uint32_t k = (n_quads << 2) + threadIdx.x; k < n_words; k += blockDim.x) dst[k] = src[k];
     g = s_gauss;
   }
   __syncthreads();
