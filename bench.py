@@ -43,6 +43,8 @@ def make_model(args, steps_total):
     m.counts_rows = steps_total + 2
     if args.cell_size:
         m.cell_size = args.cell_size
+    elif args.workload == "w0" and args.impl != "reference":
+        m.cell_size = 448      # [CFG 0]'s 5 nm cells (8 M cells for 10 k agents) are the oracle's; reading S20
     return m
 
 
