@@ -217,6 +217,58 @@ def reduce_ranks(times, work, device):
     return tt.tolist(), ww.tolist()
 
 
+def run_seeds(args):
+    """many independent seeds of one model concurrently on one GPU, one handle and one
+    CUDA stream each ("run many seeds concurrently").  Not the contract line: prints
+    the aggregate agent-steps/s of R concurrent populations next to the single-population rate."""
+    import torch
+
+    import paper_2606_14603_b200 as pkg
+
+    torch.cuda.set_device(0)
+    R, W, K = args.seeds, max(3, args.warmup), args.steps
+    base = make_model(args, W + 2 * K + 8)
+    sims = []
+    for r in range(R):
+        m = make_model(args, W + 2 * K + 8)     # the first population is timed twice
+        m.seed, m.place_seed = base.seed + 1000 * r, base.place_seed + 1000 * r
+        s = pkg.Sim(m, device="cuda:0", stream=torch.cuda.Stream())
+        s.seed_population()
+        s.step(W)
+        sims.append(s)
+    torch.cuda.synchronize()
+
+    def timed(group):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        main = torch.cuda.current_stream()
+        ev0.record(main)
+        for s in group:
+            s.stream.wait_event(ev0)
+        for s in group:
+            s.step_async(K)
+        for s in group:
+            done = torch.cuda.Event()
+            done.record(s.stream)
+            main.wait_event(done)
+        ev1.record(main)
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1)
+
+    ms_one = timed(sims[:1])
+    ms_all = timed(sims)                       # sims[0] runs K further steps: same work per step
+    work = 0.0
+    for s in sims:
+        s.step(0)
+        c = s.read_counts().astype(np.int64)
+        work += float(c[-K - 1:-1].sum())
+    one = float(sims[0].read_counts().astype(np.int64)[W:W + K].sum()) / (ms_one * 1e-3)
+    print(json.dumps({"metric": METRIC, "unit": UNIT, "value": work / (ms_all * 1e-3), "n_gpus": 1, "steps": K,
+                      "warmup": W, "ms_total": ms_all, "higher_is_better": True, "data": "synthetic", "dtype": "int32",
+                      "config": {"workload": workload_name(args, base), "concurrent_seeds": R,
+                                 "parallelism": f"{R} handles x 1 stream each on 1 GPU (no exchange)"},
+                      "single_seed_value": one, "speedup_vs_single_seed": work / (ms_all * 1e-3) / one}), flush=True)
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -397,9 +449,12 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=1)
     ap.add_argument("--ref-n", type=int, default=1_000_000, help="oracle sample size for --impl reference")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--seeds", type=int, default=1, help="N1: concurrent independent populations on one GPU (not the contract line)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.seeds > 1:
+        run_seeds(args)
     else:
         run_gpu(args)
 

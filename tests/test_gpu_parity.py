@@ -255,6 +255,27 @@ def test_w2_full_size_two_steps(gpu):
     run_both(gpu, m, 2, chunks=1)
 
 
+def test_concurrent_handles_on_separate_streams(gpu):
+    """independent seeds run concurrently, one handle + one CUDA stream each; every one of
+    them must still match its own oracle run bit for bit."""
+    import torch
+
+    models = []
+    for r in range(4):
+        m = tiny_cube(L=300 + 7 * r, n_a=900 + 50 * r, n_b=800, p_rel=0.03, seed=40 + r)
+        models.append(m)
+    sims = [gpu.Sim(m, stream=torch.cuda.Stream()) for m in models]
+    for s in sims:
+        s.seed_population()
+    for _ in range(3):                       # interleaved asynchronous stepping on four streams
+        for s in sims:
+            s.step_async(9)
+    for s, m in zip(sims, models):
+        s.step(0)
+        orc = oracle_cls()(m); orc.seed_population(); orc.step(27)
+        assert_same(s, orc, m.name)
+
+
 def test_errors(gpu):
     from paper_2606_14603_b200.binding import E_CAPACITY, E_INVAL, SimError
 
