@@ -276,6 +276,24 @@ def test_concurrent_handles_on_separate_streams(gpu):
         assert_same(s, orc, m.name)
 
 
+def test_empty_population_and_mid_run_seeding(gpu):
+    """Degenerate cases: stepping an empty handle, then adding agents mid-run (run-time treatment
+    change) with fresh ids, twice, against the oracle doing the same."""
+    m = tiny_cube(L=320, n_a=700, n_b=650, p_rel=0.02, seed=77)
+    sim = gpu.Sim(m); orc = oracle_cls()(m)
+    sim.step(3); orc.step(3)                               # nothing there yet
+    assert_same(sim, orc, "empty")
+    assert sim.info()["n_live"] == 0
+    sim.seed_population(); orc.seed_population()
+    sim.step(9); orc.step(9)
+    assert_same(sim, orc, "after first seeding")
+    extra = [SeedRecord(1, 333), SeedRecord(0, 17)]        # a dose of B and a few A, placed from another seed
+    sim.seed_population(extra, place_seed=1234); orc.seed_population(extra, place_seed=1234)
+    assert_same(sim, orc, "right after the mid-run dose")
+    sim.step(11); orc.step(11)
+    assert_same(sim, orc, "after the mid-run dose")
+
+
 def test_errors(gpu):
     from paper_2606_14603_b200.binding import E_CAPACITY, E_INVAL, SimError
 
