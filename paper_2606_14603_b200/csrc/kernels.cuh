@@ -147,61 +147,85 @@ __device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTabl
   return g;
 }
 
-// A block walks tiles of 256 x kMoveUnroll agents; every thread keeps kMoveUnroll agents in flight
+// A block walks tiles of 256 x kK1Unroll agents; every thread keeps kK1Unroll agents in flight
 // (all loads issued before the first Philox, all histogram atomics before the first rank store) so
 // that HBM and L2-atomic latency overlap.  The histogram uses warp-aggregated atomics
 // (__match_any_sync on the cell key): agents arrive nearly cell-sorted from the previous step, so a
 // warp touches few distinct cells.
-#ifndef MOLSIM_MOVE_UNROLL
-#define MOLSIM_MOVE_UNROLL 2     // tuned on B200 (W4 16M): 2 agents in flight per thread x 5 blocks/SM
+#ifndef MOLSIM_MATCH_ANY
+#define MOLSIM_MATCH_ANY 0      // 1: aggregate with __match_any_sync (measured slower)
 #endif
-#ifndef MOLSIM_MOVE_MINBLK
-#define MOLSIM_MOVE_MINBLK 5
+// Warp aggregation of the histogram atomics.  Agents arrive nearly cell-sorted from the previous
+// step, so lanes with equal keys are almost always neighbours: a run of equal keys (one shuffle, one
+// ballot) is aggregated into one atomic by its first lane.  Equal keys that are not adjacent simply
+// issue separate atomics.  (__match_any_sync finds them all but runs on the slow ADU pipe: it was
+// the top stall of this kernel.)
+__device__ __forceinline__ void run_of_key(uint32_t key, uint32_t lane, int& leader, uint32_t& rank, uint32_t& count) {
+#if MOLSIM_MATCH_ANY
+  const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
+  leader = __ffs(peers) - 1;
+  rank = __popc(peers & ((1u << lane) - 1u));
+  count = __popc(peers);
+#else
+  const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, key, 1);
+  const uint32_t heads = __ballot_sync(0xFFFFFFFFu, lane == 0u || key != prev);
+  const uint32_t upto = (2u << lane) - 1u;                        // lanes 0..lane (lane 31: all ones)
+  leader = 31 - __clz(heads & upto);
+  const uint32_t above = heads & ~upto;
+  const int end = above ? __ffs(above) - 1 : 32;
+  rank = lane - (uint32_t)leader;
+  count = (uint32_t)(end - leader);
 #endif
-constexpr int kMoveUnroll = MOLSIM_MOVE_UNROLL;
+}
+
+// Agents in flight per thread (kU) and resident blocks per SM (kB) are template parameters of K1 and
+// K3; the host picks per problem size (swept on B200: profiles/r1d_kernels.md).  Many thin blocks
+// finish a small population sooner; fewer, fatter blocks win from a few million agents on.
+struct MoveCfgSmall { static constexpr int k1u = 2, k1b = 5, k3u = 2, k3b = 5; };
+struct MoveCfgLarge { static constexpr int k1u = 4, k1b = 3, k3u = 3, k3b = 3; };
+constexpr uint32_t kLargeFrom = 2000000;   // capacity (agents) from which MoveCfgLarge is used
 constexpr int kMoveThreads = 256;
 
-template <bool kGaussSmem>
-__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_move_hist(Params p) {
+template <bool kGaussSmem, int kK1Unroll, int kMinBlk>
+__global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_move_hist(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
   const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   const uint32_t lane = threadIdx.x & 31u;
-  constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
+  constexpr uint32_t kTile = kMoveThreads * kK1Unroll;
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {   // block-uniform trip count
-    uint16_t s[kMoveUnroll];
-    int32_t x[kMoveUnroll], y[kMoveUnroll], z[kMoveUnroll];
-    uint32_t id[kMoveUnroll], key[kMoveUnroll];
+    uint16_t s[kK1Unroll];
+    int32_t x[kK1Unroll], y[kK1Unroll], z[kK1Unroll];
+    uint32_t id[kK1Unroll], key[kK1Unroll];
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK1Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
       s[a] = i < n ? p.cur.sp[i] : kDead;
     }
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK1Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
       if (i < n) { x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; }   // not gated on the species: one round trip
     }
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK1Unroll; ++a) {
       key[a] = 0xFFFFFFFFu;
       if (s[a] == kDead) continue;
       const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
       key[a] = cell_key(m.x, m.y, m.z, p);
     }
-    uint32_t first[kMoveUnroll], rank[kMoveUnroll];
-    int leader[kMoveUnroll];
+    uint32_t first[kK1Unroll], rank[kK1Unroll];
+    int leader[kK1Unroll];
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
-      const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key[a]);
-      leader[a] = __ffs(peers) - 1;
-      rank[a] = __popc(peers & ((1u << lane) - 1u));
+    for (int a = 0; a < kK1Unroll; ++a) {
+      uint32_t count;
+      run_of_key(key[a], lane, leader[a], rank[a], count);
       first[a] = 0;
-      if (s[a] != kDead && (int)lane == leader[a]) first[a] = atomicAdd(&p.cell[key[a]], (uint32_t)__popc(peers));
+      if (s[a] != kDead && (int)lane == leader[a]) first[a] = atomicAdd(&p.cell[key[a]], count);
     }
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK1Unroll; ++a) {
       const uint32_t f = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]);
       if (s[a] != kDead) p.off[base + a * kMoveThreads + threadIdx.x] = f + rank[a];
     }
@@ -279,34 +303,34 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
 // Counting-sort scatter that reorders the whole structure of arrays into cell order (a5), applying
 // phase 1 on the way (move_agent again: same result as in K1, so the same cell), and drops DEAD
 // slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
-// kMoveUnroll agents in flight per thread.  Membrane crossings change the species here; their
+// kK3Unroll agents in flight per thread.  Membrane crossings change the species here; their
 // counts deltas go straight to counts row t+1 (rare events).
-template <bool kGaussSmem>
-__global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_scatter(Params p) {
+template <bool kGaussSmem, int kK3Unroll, int kMinBlk>
+__global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
   const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
-  constexpr uint32_t kTile = kMoveThreads * kMoveUnroll;
+  constexpr uint32_t kTile = kMoveThreads * kK3Unroll;
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {
-    uint16_t s[kMoveUnroll];
-    int32_t x[kMoveUnroll], y[kMoveUnroll], z[kMoveUnroll];
-    uint32_t id[kMoveUnroll], off[kMoveUnroll];
+    uint16_t s[kK3Unroll];
+    int32_t x[kK3Unroll], y[kK3Unroll], z[kK3Unroll];
+    uint32_t id[kK3Unroll], off[kK3Unroll];
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK3Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
       s[a] = i < n ? p.cur.sp[i] : kDead;
     }
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK3Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
       if (i < n) {   // not gated on the species: one round trip
         x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; off[a] = p.off[i];
       }
     }
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK3Unroll; ++a) {
       if (s[a] == kDead) continue;
       const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
       if (m.s != s[a]) {
@@ -318,7 +342,7 @@ __global__ void __launch_bounds__(kMoveThreads, MOLSIM_MOVE_MINBLK) k_scatter(Pa
       off[a] += p.cell[cell_key(m.x, m.y, m.z, p)];
     }
 #pragma unroll
-    for (int a = 0; a < kMoveUnroll; ++a) {
+    for (int a = 0; a < kK3Unroll; ++a) {
       if (s[a] == kDead) continue;
       const uint32_t dst = off[a];
       p.oth.x[dst] = x[a]; p.oth.y[dst] = y[a]; p.oth.z[dst] = z[a];

@@ -146,6 +146,9 @@ struct sim {
   uint32_t t_host = 0;           // steps enqueued so far (the host knows t exactly)
   uint64_t launches = 0;
   int gauss_in_smem = 0;
+  void (*k_move)(Params) = nullptr;   // K1 / K3 instantiation picked at create time (Gaussian tables in shared
+  void (*k_scat)(Params) = nullptr;   // memory or not; MoveCfgSmall or MoveCfgLarge)
+  uint32_t k1_unroll = 0, k3_unroll = 0;
   size_t gauss_bytes = 0;
   uint32_t grid_move = 0, grid_scatter = 0, grid_pairs = 0, grid_uni = 0, grid_resolve = 0;
   uint32_t cell_seg = 0, scan_blocks = 1, birth_blocks = 1, tail_blocks = 1;
@@ -219,16 +222,12 @@ int enqueue_step(sim* s) {
     ProfScope ps(s, KI_CELL_ZERO, false);
     CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->run));
   }
-  { ProfScope ps(s, KI_MOVE);
-    if (s->gauss_in_smem) k_move_hist<true><<<s->grid_move, kMoveThreads, s->gauss_bytes, s->run>>>(p);
-    else k_move_hist<false><<<s->grid_move, kMoveThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_MOVE); s->k_move<<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p); }
   { ProfScope ps(s, KI_CELL_REDUCE);
     k_cell_reduce<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_CELL_SCAN);
     k_cell_scan<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
-  { ProfScope ps(s, KI_SCATTER);
-    if (s->gauss_in_smem) k_scatter<true><<<s->grid_scatter, kMoveThreads, s->gauss_bytes, s->run>>>(p);
-    else k_scatter<false><<<s->grid_scatter, kMoveThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_SCATTER); s->k_scat<<<s->grid_scatter, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p); }
   { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
@@ -397,17 +396,25 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     };
     int occ = 0;
     const size_t gsm = s->gauss_in_smem ? s->gauss_bytes : 0;
+    using S_ = MoveCfgSmall; using L_ = MoveCfgLarge;
+    const bool large = cfg->capacity >= kLargeFrom;
+    if (gsm) {
+      s->k_move = large ? k_move_hist<true, L_::k1u, L_::k1b> : k_move_hist<true, S_::k1u, S_::k1b>;
+      s->k_scat = large ? k_scatter<true, L_::k3u, L_::k3b> : k_scatter<true, S_::k3u, S_::k3b>;
+    } else {
+      s->k_move = large ? k_move_hist<false, L_::k1u, L_::k1b> : k_move_hist<false, S_::k1u, S_::k1b>;
+      s->k_scat = large ? k_scatter<false, L_::k3u, L_::k3b> : k_scatter<false, S_::k3u, S_::k3b>;
+    }
+    s->k1_unroll = large ? L_::k1u : S_::k1u; s->k3_unroll = large ? L_::k3u : S_::k3u;
     if (gsm > 48 * 1024) {
-      cudaFuncSetAttribute(k_move_hist<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
-      cudaFuncSetAttribute(k_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(s->k_move, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(s->k_scat, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
       cudaFuncSetAttribute(k_move_only<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
     }
-    if (gsm) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hist<true>, kMoveThreads, gsm);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hist<false>, kMoveThreads, 0);
-    s->grid_move = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
-    if (gsm) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter<true>, kMoveThreads, gsm);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter<false>, kMoveThreads, 0);
-    s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * kMoveUnroll);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_move, kMoveThreads, gsm);
+    s->grid_move = sized(occ, (uint64_t)kMoveThreads * s->k1_unroll);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_scat, kMoveThreads, gsm);
+    s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * s->k3_unroll);
     s->grid_pairs = (uint32_t)(((uint64_t)cfg->capacity + kPairThreads - 1) / kPairThreads);   // one tile per block
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, kUniThreads, 0);
     s->grid_uni = sized(occ, kUniTile);

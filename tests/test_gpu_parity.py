@@ -223,6 +223,20 @@ def test_w4_200k_and_step_split(gpu):
         assert (a[k] == c[k]).all()
 
 
+def test_large_capacity_kernel_configuration(gpu):
+    """K1/K3 are instantiated with more agents per thread from a capacity of 2 M agents on (MoveCfgLarge);
+    the same small populations must give the same result through that instantiation (ragged tiles, a sphere
+    with membrane crossings, and a cube)."""
+    m = configs.w4(n=150_003, n_steps=12)
+    m.capacity = 2_100_000
+    m.finalize()
+    run_both(gpu, m, 12, chunks=2)
+    m = configs.w3(scale=0.004, n_steps=60)
+    m.capacity = 2_100_000
+    m.finalize()
+    run_both(gpu, m, 60, chunks=2)
+
+
 def test_w4_1m_full_size_steps(gpu):
     """[CFG 4] N = 1 M in the bench launch configuration, 6 steps, full state compare."""
     m = configs.w4(n=1_000_000, n_steps=6)
