@@ -13,6 +13,8 @@ constexpr int kMaxSpecies = 64;
 constexpr int kMaxReactions = 64;
 constexpr int kMaxCompartments = 8;
 constexpr int kMaxRules = 8;
+constexpr uint32_t kMidShift = 8;     // birth_mid: newborn counts per 2^8 parent ids
+constexpr uint32_t kMaxTop = 2048;     // birth_top: entries (per 2^top_shift parent ids)
 
 enum : uint32_t { kTagMove = 1, kTagPair = 2, kTagUni = 3, kTagBirth = 4, kTagPlace = 5 };
 enum : uint8_t { kChNone = 0, kChBirth = 1, kChRelease = 2, kChConvert = 3, kChDegrade = 4, kChDelayed = 5 };
@@ -69,7 +71,9 @@ struct Params {
   uint32_t* cell;           // [n_cells + 1]: counts, then exclusive starts; cell[n_cells] = n_sorted
   uint32_t* partial;        // scan partials
   uint32_t* bits;           // birth bitmap, 4 bits per id
-  uint32_t* chunk_prefix;   // exclusive newborn prefix per 64-id chunk
+  uint32_t* birth_mid;      // newborns of this step per block of 256 parent ids
+  uint32_t* birth_top;      // newborns of this step per 2^top_shift parent ids (<= 2048 entries)
+  uint32_t top_shift;
   uint2* birth_list;        // (parent slot, mask | pre-species << 16)
   uint32_t* counts;         // [counts_rows][n_replicas][n_species]
   Scalars* scal;

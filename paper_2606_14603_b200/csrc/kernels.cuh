@@ -682,6 +682,8 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
   if (mask) {
     for (uint32_t k = 0; k < 4u; ++k) if (mask >> k & 1u) atomicAdd(&d[S.ch[k].prod1], 1);
     atomicOr(&p.bits[id >> 3], mask << ((id & 7u) * 4u));
+    atomicAdd(&p.birth_mid[id >> kMidShift], (uint32_t)__popc(mask));     // newborn counts per 256 ids and per
+    atomicAdd(&p.birth_top[id >> p.top_shift], (uint32_t)__popc(mask));   // 2^top_shift ids: K6 ranks from these
     const uint32_t e = atomicAdd(&p.scal->birth_count, 1u);
     p.birth_list[e] = make_uint2(i, mask | ((uint32_t)s0 << 16));
   }
@@ -754,79 +756,64 @@ __global__ void __launch_bounds__(kUniThreads) k_uni(Params p) {
   delta_flush(s_delta, p.counts + (size_t)(t + 1) * p.row_width, p.row_width);
 }
 
-// ----------------------------------------------------------------------------- K6 birth ranking
-// New ids are assigned in (parent id, channel) order (north_star (5), S14): the birth bitmap is
-// indexed by parent id, so a newborn's rank is the popcount of all lower bits.  Two launches
-// (segment sums, then per-64-id-chunk exclusive prefixes); both return at once on steps without births.
-__device__ __forceinline__ uint32_t chunk_popc(const uint32_t* __restrict__ bits, uint32_t c) {
-  const uint4 a = *reinterpret_cast<const uint4*>(bits + (size_t)c * 8u);
-  const uint4 b = *reinterpret_cast<const uint4*>(bits + (size_t)c * 8u + 4u);
-  return __popc(a.x) + __popc(a.y) + __popc(a.z) + __popc(a.w) + __popc(b.x) + __popc(b.y) + __popc(b.z) + __popc(b.w);
-}
-
-__global__ void __launch_bounds__(kScanThreads) k_birth_reduce(Params p) {
+// ----------------------------------------------------------------------------- K6 births
+// New ids are assigned in (parent id, channel) order (north_star (5), S14).  The birth bitmap (4 bits
+// per id) is indexed by parent id, so a newborn's rank is the number of set bits below its own; K5
+// also keeps the newborn count of every block of 256 ids (birth_mid) and of every 2^top_shift ids
+// (birth_top, at most kMaxTop entries).  One launch: every block scans birth_top into shared memory,
+// then one warp per firing parent adds the birth_mid entries and bitmap words between the block
+// boundaries and the parent (a few dozen coalesced loads per lane at most) and lanes 0..3 place the
+// newborns (phase 4, a9): newborn g of the step gets id next_id + g and slot n_sorted + g.
+__global__ void __launch_bounds__(kScanThreads) k_births(Params p) {
   __shared__ uint32_t s_warp[9];
-  if (p.scal->birth_count == 0) return;
-  const uint32_t n_chunks = (p.scal->next_id + 63u) >> 6;
-  const uint32_t seg = ((n_chunks + gridDim.x - 1) / gridDim.x + kScanThreads - 1) / kScanThreads * kScanThreads;
-  const uint32_t lo = min(blockIdx.x * seg, n_chunks), hi = min(lo + seg, n_chunks);
-  uint32_t sum = 0;
-  for (uint32_t c = lo + threadIdx.x; c < hi; c += kScanThreads) sum += chunk_popc(p.bits, c);
-  const uint32_t tot = block_sum(sum, s_warp);
-  if (threadIdx.x == 0) p.partial[blockIdx.x] = tot;
-}
-
-__global__ void __launch_bounds__(kScanThreads) k_birth_scan(Params p) {
-  __shared__ uint32_t s_warp[9];
-  if (p.scal->birth_count == 0) {
+  __shared__ uint32_t s_top[kMaxTop];
+  const uint32_t nb = p.scal->birth_count;
+  if (nb == 0) {
     if (blockIdx.x == 0 && threadIdx.x == 0) p.scal->total_births = 0;
     return;
   }
-  const uint32_t n_chunks = (p.scal->next_id + 63u) >> 6;
-  const uint32_t seg = ((n_chunks + gridDim.x - 1) / gridDim.x + kScanThreads - 1) / kScanThreads * kScanThreads;
-  const uint32_t lo = min(blockIdx.x * seg, n_chunks), hi = min(lo + seg, n_chunks);
-  uint32_t mine = 0;
-  for (uint32_t b = threadIdx.x; b < blockIdx.x; b += kScanThreads) mine += p.partial[b];
-  uint32_t running = block_sum(mine, s_warp);
-  for (uint32_t tile = lo; tile < hi; tile += kScanThreads) {
-    const uint32_t c = tile + threadIdx.x;
-    const uint32_t v = c < hi ? chunk_popc(p.bits, c) : 0u;
-    uint32_t total;
-    const uint32_t e = running + block_excl_scan(v, total, s_warp);
-    if (c < hi) p.chunk_prefix[c] = e;
-    running += total;
-  }
-  if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) p.scal->total_births = running;
-}
-
-// Phase 4: newborn placement, id assignment and append (a9).  Newborn g of the step gets
-// id next_id + g and slot n_sorted + g.
-__global__ void __launch_bounds__(128) k_births(Params p) {
-  const uint32_t nb = p.scal->birth_count;
-  if (nb == 0) return;
-  const uint32_t n_sorted = p.cell[p.n_cells], total = p.scal->total_births;
   const uint32_t next_id = p.scal->next_id, t = p.scal->t;
+  const uint32_t n_top = ((next_id - 1u) >> p.top_shift) + 1u;          // parents have ids < next_id
+  constexpr uint32_t kPer = kMaxTop / kScanThreads;
+  uint32_t v[kPer], sum = 0;
+#pragma unroll
+  for (uint32_t k = 0; k < kPer; ++k) {
+    const uint32_t j = threadIdx.x * kPer + k;
+    v[k] = j < n_top ? p.birth_top[j] : 0u;
+    sum += v[k];
+  }
+  uint32_t total;
+  uint32_t e0 = block_excl_scan(sum, total, s_warp);
+#pragma unroll
+  for (uint32_t k = 0; k < kPer; ++k) { s_top[threadIdx.x * kPer + k] = e0; e0 += v[k]; }
+  __syncthreads();
+  const uint32_t n_sorted = p.cell[p.n_cells];
   uint32_t bad = 0;
   if ((unsigned long long)n_sorted + total > p.capacity) bad |= 1u;
   if ((unsigned long long)next_id + total > p.id_capacity) bad |= 2u;
-  if (bad) {
-    if (blockIdx.x == 0 && threadIdx.x == 0) atomicOr(&p.scal->err, bad);
-    return;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    p.scal->total_births = total;
+    if (bad) atomicOr(&p.scal->err, bad);
   }
+  if (bad) return;
   const DevTables* __restrict__ T = p.tab;
-  const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < nb; e += stride) {
+  const uint32_t lane = threadIdx.x & 31u, wpb = kScanThreads / 32;
+  for (uint32_t e = blockIdx.x * wpb + (threadIdx.x >> 5); e < nb; e += gridDim.x * wpb) {
     const uint2 ent = p.birth_list[e];
     const uint32_t slot = ent.x, mask = ent.y & 0xFu, pre = ent.y >> 16;
     const uint32_t pid = p.oth.id[slot];
-    const int32_t px = p.oth.x[slot], py = p.oth.y[slot], pz = p.oth.z[slot];
-    uint32_t rank = p.chunk_prefix[pid >> 6];
-    for (uint32_t w = (pid >> 6) * 8u; w < (pid >> 3); ++w) rank += __popc(p.bits[w]);
-    rank += __popc(p.bits[pid >> 3] & ((1u << ((pid & 7u) * 4u)) - 1u));
-    const int32_t rbase = (int32_t)(((uint32_t)px >> p.stride_shift) << p.stride_shift);
-    const int32_t lx = px - rbase;
-    for (uint32_t k = 0; k < 4u; ++k) {
-      if (!(mask >> k & 1u)) continue;
+    uint32_t part = 0;
+    for (uint32_t j = ((pid >> p.top_shift) << (p.top_shift - kMidShift)) + lane; j < (pid >> kMidShift); j += 32u)
+      part += p.birth_mid[j];
+    const uint32_t w0 = (pid >> kMidShift) << (kMidShift - 3u), w1 = pid >> 3;      // bitmap words of this 256-id block
+    if (w0 + lane < w1) part += __popc(p.bits[w0 + lane]);
+    if (lane == 31u) part += __popc(p.bits[w1] & ((1u << ((pid & 7u) * 4u)) - 1u));
+    const uint32_t rank0 = s_top[pid >> p.top_shift] + __reduce_add_sync(0xFFFFFFFFu, part);
+    if (lane < 4u && (mask >> lane & 1u)) {
+      const uint32_t k = lane, rank = rank0 + __popc(mask & ((1u << k) - 1u));
+      const int32_t px = p.oth.x[slot], py = p.oth.y[slot], pz = p.oth.z[slot];
+      const int32_t rbase = (int32_t)(((uint32_t)px >> p.stride_shift) << p.stride_shift);
+      const int32_t lx = px - rbase;
       const uint16_t sp_new = T->sp[pre].ch[k].prod1;
       const uint4 r = philox_sim(p, pid, k, t, kTagBirth);
       int32_t qx = lx + (int32_t)__umulhi(r.x, 21u) - 10;
@@ -839,13 +826,12 @@ __global__ void __launch_bounds__(128) k_births(Params p) {
       p.oth.x[dst] = qx + rbase; p.oth.y[dst] = qy; p.oth.z[dst] = qz;
       p.oth.id[dst] = next_id + rank;
       p.oth.sp[dst] = sp_new;
-      ++rank;
     }
   }
 }
 
 // ----------------------------------------------------------------------------- K7 epilogue
-// Clears the touched birth-bitmap words; the last block to finish advances the device scalars and
+// Clears the touched birth-bitmap words and counters; the last block to finish advances the device scalars and
 // seeds counts row t+2 with row t+1 (the next step adds its deltas to it; a10).
 __global__ void __launch_bounds__(256) k_epilogue(Params p) {
   __shared__ uint32_t s_last;
@@ -853,7 +839,7 @@ __global__ void __launch_bounds__(256) k_epilogue(Params p) {
   const uint32_t stride = gridDim.x * blockDim.x;
   for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < nb; e += stride) {
     const uint32_t pid = p.oth.id[p.birth_list[e].x];
-    p.bits[pid >> 3] = 0u;
+    p.bits[pid >> 3] = 0u; p.birth_mid[pid >> kMidShift] = 0u; p.birth_top[pid >> p.top_shift] = 0u;
   }
   __threadfence();
   __syncthreads();

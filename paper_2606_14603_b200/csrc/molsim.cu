@@ -16,19 +16,18 @@ using namespace molsim;
 namespace {
 
 constexpr uint32_t kMaxScanBlocks = 592;  // 148 SMs x 4; small problems get proportionally smaller grids (launch-bound)
-constexpr uint32_t kMaxBirthBlocks = 296; // 148 SMs x 2
 constexpr uint32_t kMaxTailBlocks = 148;
 
 enum KernelId { KI_MOVE = 0, KI_CELL_ZERO, KI_CELL_REDUCE, KI_CELL_SCAN, KI_SCATTER, KI_PAIRS,
-                KI_RESOLVE, KI_UNI, KI_BIRTH_REDUCE, KI_BIRTH_SCAN, KI_BIRTHS, KI_EPILOGUE, KI_OTHER };
+                KI_RESOLVE, KI_UNI, KI_BIRTHS, KI_EPILOGUE, KI_OTHER };
 const char* kKernelNames[SIM_N_KERNELS] = {
     "k_move_hist", "memset_cells", "k_cell_reduce", "k_cell_scan", "k_scatter", "k_pairs",
-    "k_resolve", "k_uni", "k_birth_reduce", "k_birth_scan", "k_births", "k_epilogue", "other"};
+    "k_resolve", "k_uni", "k_births", "k_epilogue", "other"};
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t soa[2][5], off, prop, best, hasprop, cell, partial, bits, chunk_prefix, birth_list, counts,
+  size_t soa[2][5], off, prop, best, hasprop, cell, partial, bits, birth_mid, birth_top, birth_list, counts,
       scal, tab, gauss, total;
   uint32_t n_cells, nx, ny, nz;
 };
@@ -50,7 +49,8 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   L.partial = take(4096 * 4);
   const size_t n_chunks = ((size_t)c->id_capacity + 63) / 64 + 1;
   L.bits = take(n_chunks * 8 * 4);
-  L.chunk_prefix = take(n_chunks * 4);
+  L.birth_mid = take((((size_t)c->id_capacity >> kMidShift) + 2) * 4);
+  L.birth_top = take((size_t)kMaxTop * 4);
   L.birth_list = take(cap * 8);
   L.counts = take(((size_t)c->counts_rows + 2) * c->n_replicas * c->n_species * 4);
   L.scal = take(sizeof(Scalars));
@@ -151,7 +151,7 @@ struct sim {
   uint32_t k1_unroll = 0, k3_unroll = 0;
   size_t gauss_bytes = 0;
   uint32_t grid_move = 0, grid_scatter = 0, grid_pairs = 0, grid_uni = 0, grid_resolve = 0;
-  uint32_t cell_seg = 0, scan_blocks = 1, birth_blocks = 1, tail_blocks = 1;
+  uint32_t cell_seg = 0, scan_blocks = 1, tail_blocks = 1;
   bool profile = false;
   float prof_ms[SIM_N_KERNELS] = {};
   uint32_t prof_n[SIM_N_KERNELS] = {};
@@ -231,9 +231,7 @@ int enqueue_step(sim* s) {
   { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_BIRTH_REDUCE); k_birth_reduce<<<s->birth_blocks, kScanThreads, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_BIRTH_SCAN); k_birth_scan<<<s->birth_blocks, kScanThreads, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_BIRTHS); k_births<<<s->tail_blocks, 128, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_BIRTHS); k_births<<<s->tail_blocks, kScanThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_EPILOGUE); k_epilogue<<<s->tail_blocks, 256, 0, s->run>>>(p); }
   CK(cudaGetLastError());
   std::swap(p.cur, p.oth);   // the sorted copy (+ newborns) is the next step's current state
@@ -358,7 +356,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   p.off = (uint32_t*)(w + L.off); p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
   p.best = (unsigned long long*)(w + L.best);
   p.cell = (uint32_t*)(w + L.cell); p.partial = (uint32_t*)(w + L.partial);
-  p.bits = (uint32_t*)(w + L.bits); p.chunk_prefix = (uint32_t*)(w + L.chunk_prefix);
+  p.bits = (uint32_t*)(w + L.bits); p.birth_mid = (uint32_t*)(w + L.birth_mid); p.birth_top = (uint32_t*)(w + L.birth_top);
   p.birth_list = (uint2*)(w + L.birth_list); p.counts = (uint32_t*)(w + L.counts);
   p.scal = (Scalars*)(w + L.scal); p.tab = (const DevTables*)(w + L.tab); p.gauss = (const int16_t*)(w + L.gauss);
   p.key0 = (uint32_t)cfg->seed; p.key1 = (uint32_t)(cfg->seed >> 32);
@@ -382,6 +380,8 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   p.max_r = (int32_t)std::ceil(std::sqrt((double)max_r2));
   while ((uint64_t)p.max_r * p.max_r < max_r2) p.max_r++;
   p.row_width = cfg->n_replicas * cfg->n_species;
+  p.top_shift = 16;                                                   // birth_top: at most kMaxTop entries
+  while ((((uint64_t)cfg->id_capacity - 1) >> p.top_shift) + 1 > kMaxTop) p.top_shift++;
 
   s->gauss_bytes = ((size_t)cfg->n_sigma_classes << cfg->table_bits) * 2;
   s->gauss_in_smem = s->gauss_bytes <= 160 * 1024;
@@ -425,14 +425,13 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   auto clampu = [](uint64_t v, uint64_t lo, uint64_t hi) { return (uint32_t)std::min(std::max(v, lo), hi); };
   s->scan_blocks = clampu(((uint64_t)L.n_cells + 4095) / 4096, 1, kMaxScanBlocks);          // >= 4 K cells per block
   s->cell_seg = (uint32_t)align_up(((size_t)L.n_cells + s->scan_blocks - 1) / s->scan_blocks, 1024);
-  s->birth_blocks = clampu(((uint64_t)cfg->id_capacity / 64 + 4095) / 4096, 1, kMaxBirthBlocks);  // >= 4 K id chunks per block
   s->tail_blocks = clampu(((uint64_t)cfg->capacity + 65535) / 65536, 2, kMaxTailBlocks);
 
   Scalars sc;
   std::memset(&sc, 0, sizeof(sc));
   for (int r = 0; r < kMaxRules; ++r) sc.t_first[r] = kNever;
   bool ok = true;
-  ok = ok && cudaMemsetAsync(p.bits, 0, L.chunk_prefix - L.bits, s->stream) == cudaSuccess;
+  ok = ok && cudaMemsetAsync(p.bits, 0, L.birth_list - L.bits, s->stream) == cudaSuccess;
   ok = ok && cudaMemsetAsync(p.best, 0xFF, L.hasprop - L.best, s->stream) == cudaSuccess;
   ok = ok && cudaMemsetAsync(p.hasprop, 0, L.cell - L.hasprop, s->stream) == cudaSuccess;
   ok = ok && cudaMemsetAsync(p.counts, 0, L.scal - L.counts, s->stream) == cudaSuccess;
