@@ -110,7 +110,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
 int sim_seed_population(sim_t*, const sim_seed_rec_t* recs, uint32_t n_recs, uint64_t place_seed);
 
 /* Advances n_steps time steps (DESIGN.md §1 phases 1-6 per step).  All work is enqueued on the
- * stream without host synchronisation between steps (the 12 launches of a step are replayed as
+ * stream without host synchronisation between steps (the 10 launches of a step are replayed as
  * CUDA graphs captured once per handle); the call then waits for the stream once and
  * returns the sticky device error state (capacity / id space), if any.  Handles are independent:
  * several may step concurrently on different streams ("many seeds per GPU"). */
@@ -156,6 +156,53 @@ const char* sim_kernel_name(int k);
 void sim_destroy(sim_t*);
 const char* sim_strerror(int code);
 const char* sim_last_cuda_error(const sim_t*);
+
+/* ---- read-outs next to the step ------------------------------- */
+
+/* Threshold monitor over a window of the per-step counts log, evaluated on the device (PAPER.md:58:
+ * "designate specific molecular species for continuous monitoring ... concentration thresholds within
+ * specified time windows"; Fig. 2: the cell state switches between Cancerous and Normal as
+ * the monitored species crosses the threshold).  Reading S24: value(t) = sum over `species` of
+ * counts[t][replica][s]; above(t) = value(t) > threshold (a concentration threshold is converted to a
+ * count by the caller, n = c N_A V). */
+typedef struct {
+  uint32_t replica;
+  uint32_t n_species;          /* 1..4 */
+  uint16_t species[4];
+  uint32_t threshold;
+  uint32_t first_row, n_rows;  /* window: counts rows first_row .. first_row+n_rows-1, all <= steps done */
+} sim_monitor_t;
+typedef struct {
+  uint32_t first_above;        /* first row of the window with above(t), 0xFFFFFFFF if none */
+  uint32_t n_above;            /* rows of the window with above(t) */
+  uint32_t last_state;         /* above(last row): 1 = over the threshold ("Cancerous" in Fig. 2), 0 = "Normal" */
+  uint32_t max_value, max_row; /* maximum of value(t) over the window and the first row that attains it */
+  uint32_t n_switches;         /* rows t > first_row of the window with above(t) != above(t-1) */
+} sim_monitor_result_t;
+/* mons[n_mons] and out[n_mons] are HOST arrays (n_mons <= 64).  states may be NULL; else HOST bytes,
+ * above(t) of monitor m at states[m * states_stride + (t - first_row)], states_stride >= every n_rows.
+ * SIM_E_INVAL: bad replica / species / empty window / window beyond the steps done.  Synchronises. */
+int sim_monitor_eval(sim_t*, const sim_monitor_t* mons, uint32_t n_mons, sim_monitor_result_t* out,
+                     uint8_t* states, uint32_t states_stride);
+
+/* Headless stand-in for the paper's 3-D viewer (Fig. 1: molecules highlighted by
+ * compartment, orange for cytoplasm, yellow for nucleus): orthographic point splat of the live agents of
+ * one replica into an RGBA8 image, computed on the device and copied to `rgba` (HOST,
+ * height*width*4 bytes, row 0 = smallest v).  Reading S25: the image plane holds the two axes other than
+ * `axis` in increasing order (u, v); an agent with u0 <= u < u0+eu, v0 <= v < v0+ev (local coordinates)
+ * falls into pixel ((u-u0)*width / eu, (v-v0)*height / ev); per pixel and compartment c the agents are
+ * counted (n_c); channel k = min(255, sum_c palette[c][k] * min(n_c*gain, 255) / 255); alpha = 255 where
+ * any agent fell, else 0.  Uses scratch of the handle that is free between steps.
+ * SIM_E_INVAL: bad view, or width*height*n_compartments > 2*capacity / width*height > capacity. */
+typedef struct {
+  uint32_t replica, axis;      /* axis 0, 1, 2 = projected away */
+  int32_t u0, v0;
+  uint32_t eu, ev;             /* window extent in units (> 0) */
+  uint32_t width, height;      /* pixels (> 0) */
+  uint32_t gain;               /* 1..255 */
+  uint8_t palette[SIM_MAX_COMPARTMENTS][4];   /* r, g, b, unused, per compartment index */
+} sim_view_t;
+int sim_render(sim_t*, const sim_view_t* view, uint8_t* rgba);
 
 /* Test hook: Philox4x32-10 on the device for n (counter,key) pairs; DEVICE pointers
  * ctr[4n], key[2n], out[4n]; enqueued on `cuda_stream`. */

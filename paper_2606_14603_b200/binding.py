@@ -49,7 +49,7 @@ class _Config(C.Structure):
 EXPORTS = ["sim_workspace_bytes", "sim_create", "sim_seed_population", "sim_step", "sim_step_async",
            "sim_read_counts", "sim_read_agents", "sim_load_agents", "sim_info", "sim_debug_move_only",
            "sim_launch_count", "sim_profile_enable", "sim_kernel_times", "sim_kernel_name", "sim_destroy",
-           "sim_strerror", "sim_last_cuda_error", "sim_debug_philox"]
+           "sim_strerror", "sim_last_cuda_error", "sim_debug_philox", "sim_monitor_eval", "sim_render"]
 
 _lib = None
 
@@ -88,8 +88,26 @@ def load_library():
     L.sim_last_cuda_error.argtypes = [vp]
     L.sim_last_cuda_error.restype = C.c_char_p
     L.sim_debug_philox.argtypes = [vp, vp, vp, u32, vp]
+    L.sim_monitor_eval.argtypes = [vp, vp, u32, vp, vp, u32]
+    L.sim_render.argtypes = [vp, vp, vp]
     _lib = L
     return L
+
+
+class _Monitor(C.Structure):
+    _fields_ = [("replica", C.c_uint32), ("n_species", C.c_uint32), ("species", C.c_uint16 * 4),
+                ("threshold", C.c_uint32), ("first_row", C.c_uint32), ("n_rows", C.c_uint32)]
+
+
+class _MonitorResult(C.Structure):
+    _fields_ = [("first_above", C.c_uint32), ("n_above", C.c_uint32), ("last_state", C.c_uint32),
+                ("max_value", C.c_uint32), ("max_row", C.c_uint32), ("n_switches", C.c_uint32)]
+
+
+class _View(C.Structure):
+    _fields_ = [("replica", C.c_uint32), ("axis", C.c_uint32), ("u0", C.c_int32), ("v0", C.c_int32),
+                ("eu", C.c_uint32), ("ev", C.c_uint32), ("width", C.c_uint32), ("height", C.c_uint32),
+                ("gain", C.c_uint32), ("palette", (C.c_uint8 * 4) * 8)]
 
 
 class SimError(RuntimeError):
@@ -234,6 +252,45 @@ class Sim:
         n = np.zeros(N_KERNELS, dtype=np.uint32)
         self._check(self._lib.sim_kernel_times(self._h, _ptr(ms), _ptr(n)))
         return {self._lib.sim_kernel_name(k).decode(): (float(ms[k]), int(n[k])) for k in range(N_KERNELS)}
+
+    def monitor_eval(self, monitors, with_states=True):
+        """monitors: dicts {replica, species (1..4 ids), threshold, first_row, n_rows}; sim_monitor_eval."""
+        n = len(monitors)
+        mons = (_Monitor * max(n, 1))()
+        for i, m in enumerate(monitors):
+            mons[i].replica, mons[i].n_species = m["replica"], len(m["species"])
+            for k, sp in enumerate(m["species"][:4]):
+                mons[i].species[k] = sp
+            mons[i].threshold, mons[i].first_row, mons[i].n_rows = m["threshold"], m["first_row"], m["n_rows"]
+        res = (_MonitorResult * max(n, 1))()
+        stride = max([m["n_rows"] for m in monitors] + [1])
+        states = np.zeros((max(n, 1), stride), dtype=np.uint8)
+        self._check(self._lib.sim_monitor_eval(self._h, mons, n, res, _ptr(states) if with_states else None, stride))
+        out = []
+        for i, m in enumerate(monitors):
+            d = {k: int(getattr(res[i], k)) for k, _ in _MonitorResult._fields_}
+            if with_states:
+                d["states"] = states[i, :m["n_rows"]].copy()
+            out.append(d)
+        return out
+
+
+    def render(self, replica=0, axis=2, u0=0, v0=0, eu=None, ev=None, width=256, height=256, gain=255, palette=None):
+        """RGBA8 picture of the live agents of one replica, coloured by compartment; sim_render."""
+        ext = [e for a, e in enumerate(self.model.extent) if a != axis]
+        if axis != 0 and self.model.n_replicas > 1:
+            ext[0] = min(ext[0], 1 << self.model.stride_shift)
+        v = _View()
+        v.replica, v.axis, v.u0, v.v0 = replica, axis, u0, v0
+        v.eu, v.ev = (ext[0] if eu is None else eu), (ext[1] if ev is None else ev)
+        v.width, v.height, v.gain = width, height, gain
+        palette = palette or [(255, 165, 0), (255, 255, 0)]     # PAPER.md:68: cytoplasm orange, nucleus yellow
+        for c in range(min(8, len(palette))):
+            for k in range(3):
+                v.palette[c][k] = palette[c][k]
+        img = np.zeros((height, width, 4), dtype=np.uint8)
+        self._check(self._lib.sim_render(self._h, C.byref(v), _ptr(img)))
+        return img
 
 
 def debug_philox(ctr, key):

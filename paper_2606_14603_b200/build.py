@@ -6,6 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "libmolsim.so")
 SRC = os.path.join(HERE, "csrc", "molsim.cu")
 DEPS = [SRC, os.path.join(HERE, "csrc", "kernels.cuh"), os.path.join(HERE, "csrc", "device_types.cuh"),
+        os.path.join(HERE, "csrc", "readout.cuh"),
         os.path.join(os.path.dirname(HERE), "include", "molsim.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 

@@ -3,6 +3,7 @@
 // hot path runs in the kernels of kernels.cuh; there is no CPU fallback.
 #include "../../include/molsim.h"
 #include "kernels.cuh"
+#include "readout.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -674,6 +675,74 @@ const char* sim_strerror(int code) {
 }
 
 const char* sim_last_cuda_error(const sim_t* s) { return s ? s->cuda_err.c_str() : ""; }
+
+int sim_monitor_eval(sim_t* s, const sim_monitor_t* mons, uint32_t n_mons, sim_monitor_result_t* out,
+                     uint8_t* states, uint32_t states_stride) {
+  if (!s || !mons || !out || n_mons == 0 || n_mons > 64) return SIM_E_INVAL;
+  if (s->sticky) return s->sticky;
+  std::vector<DevMonitor> dm(n_mons);
+  for (uint32_t m = 0; m < n_mons; ++m) {
+    const sim_monitor_t& a = mons[m];
+    if (a.replica >= s->cfg.n_replicas || a.n_species == 0 || a.n_species > 4 || a.n_rows == 0) return SIM_E_INVAL;
+    if ((uint64_t)a.first_row + a.n_rows > (uint64_t)s->t_host + 1) return SIM_E_INVAL;   // rows not simulated yet
+    if (states && a.n_rows > states_stride) return SIM_E_INVAL;
+    DevMonitor& d = dm[m];
+    d.replica = a.replica; d.n_species = a.n_species; d.threshold = a.threshold;
+    d.first_row = a.first_row; d.n_rows = a.n_rows; d.states_off = m * states_stride;
+    for (uint32_t k = 0; k < 4; ++k) {
+      if (k < a.n_species && a.species[k] >= s->cfg.n_species) return SIM_E_INVAL;
+      d.species[k] = k < a.n_species ? a.species[k] : 0;
+    }
+  }
+  // scratch: the birth list is free between steps
+  const size_t state_bytes = states ? (size_t)n_mons * states_stride : 0;
+  if (8192 + state_bytes > (size_t)s->cfg.capacity * 8) return SIM_E_INVAL;
+  char* scratch = (char*)s->prm.birth_list;
+  DevMonitor* d_mon = (DevMonitor*)scratch;
+  DevMonitorResult* d_res = (DevMonitorResult*)(scratch + 4096);
+  uint8_t* d_states = states ? (uint8_t*)(scratch + 8192) : nullptr;
+  CK(cudaMemcpyAsync(d_mon, dm.data(), n_mons * sizeof(DevMonitor), cudaMemcpyHostToDevice, s->stream));
+  if (d_states) CK(cudaMemsetAsync(d_states, 0, state_bytes, s->stream));
+  { ProfScope ps(s, KI_OTHER);
+    k_monitor<<<n_mons, kMonThreads, 0, s->stream>>>(s->prm.counts, s->prm.row_width, s->prm.n_species, d_mon, d_res, d_states); }
+  CK(cudaGetLastError());
+  static_assert(sizeof(DevMonitorResult) == sizeof(sim_monitor_result_t), "result layout");
+  CK(cudaMemcpyAsync(out, d_res, n_mons * sizeof(DevMonitorResult), cudaMemcpyDeviceToHost, s->stream));
+  if (d_states) CK(cudaMemcpyAsync(states, d_states, state_bytes, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return SIM_OK;
+}
+
+int sim_render(sim_t* s, const sim_view_t* view, uint8_t* rgba) {
+  if (!s || !view || !rgba) return SIM_E_INVAL;
+  if (s->sticky) return s->sticky;
+  const sim_view_t& a = *view;
+  if (a.replica >= s->cfg.n_replicas || a.axis > 2 || a.eu == 0 || a.ev == 0 || a.width == 0 || a.height == 0 ||
+      a.gain == 0 || a.gain > 255 || a.eu > 0x7FFFFFFFu || a.ev > 0x7FFFFFFFu)
+    return SIM_E_INVAL;
+  const uint64_t n_pix = (uint64_t)a.width * a.height, n_comp = s->cfg.n_compartments;
+  if (n_pix > s->cfg.capacity || n_pix * n_comp > 2ull * s->cfg.capacity) return SIM_E_INVAL;
+  DevView v;
+  v.replica = a.replica; v.axis = a.axis; v.u0 = a.u0; v.v0 = a.v0; v.eu = a.eu; v.ev = a.ev;
+  v.width = a.width; v.height = a.height; v.gain = a.gain; v.n_comp = (uint32_t)n_comp;
+  std::memcpy(v.palette, a.palette, sizeof(v.palette));
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  uint32_t* d_cnt = (uint32_t*)s->prm.birth_list;      // scratch that is free between steps
+  uchar4* d_img = (uchar4*)s->prm.off;
+  CK(cudaMemsetAsync(d_cnt, 0, n_pix * n_comp * 4, s->stream));
+  if (sc.n_slots) {
+    ProfScope ps(s, KI_OTHER);
+    k_splat_count<<<std::min<uint32_t>((sc.n_slots + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, v, sc.n_slots, d_cnt);
+  }
+  { ProfScope ps(s, KI_OTHER);
+    k_splat_colour<<<(uint32_t)std::min<uint64_t>((n_pix + 255) / 256, 148 * 8), 256, 0, s->stream>>>(v, d_cnt, d_img); }
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(rgba, d_img, n_pix * 4, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return SIM_OK;
+}
 
 int sim_debug_philox(const uint32_t* d_ctr, const uint32_t* d_key, uint32_t* d_out, uint32_t n, void* cuda_stream) {
   if (!d_ctr || !d_key || !d_out) return SIM_E_INVAL;
