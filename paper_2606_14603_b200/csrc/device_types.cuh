@@ -65,6 +65,7 @@ struct Params {
   Soa cur, oth;             // cur: state at step start (moved in place); oth: cell-sorted copy,
                             // on which bind / unimolecular / births act in place
   uint32_t* off;            // within-cell rank from the histogram pass
+  uint32_t* disp;           // accepted displacement of this step, 3 x 10 bits + crossing flag (K1 -> K3)
   unsigned long long* best; // proposal key (dist^2 << 32 | partner id) per sorted slot, ~0 = none
   uint32_t* prop;           // slot of the partner that last lowered best[i] (checked against the key in K4b)
   uint32_t* hasprop;        // 1 bit per sorted slot: best[i] was touched this step (cleared by K5)

@@ -186,7 +186,16 @@ struct MoveCfgLarge { static constexpr int k1u = 4, k1b = 3, k3u = 3, k3b = 3; }
 constexpr uint32_t kLargeFrom = 2000000;   // capacity (agents) from which MoveCfgLarge is used
 constexpr int kMoveThreads = 256;
 
-template <bool kGaussSmem, int kK1Unroll, int kMinBlk>
+// kPack: the accepted displacement (|d| <= 511 on every axis: validated by the host from the tables) and the
+// membrane-crossing flag are also written, packed into one 32-bit word per agent, so that K3 re-applies the move
+// with three adds instead of a second Philox + table + boundary evaluation.  Used while the state is
+// L2-resident (small populations); at 16 M agents the extra 4 B/agent stream costs more than the arithmetic.
+__device__ __forceinline__ uint32_t pack_disp(int32_t dx, int32_t dy, int32_t dz, bool crossed) {
+  return ((uint32_t)dx & 0x3FFu) | (((uint32_t)dy & 0x3FFu) << 10) | (((uint32_t)dz & 0x3FFu) << 20) | ((uint32_t)crossed << 30);
+}
+__device__ __forceinline__ int32_t unpack10(uint32_t w, uint32_t shift) { return (int32_t)(w << (22u - shift)) >> 22; }
+
+template <bool kGaussSmem, int kK1Unroll, int kMinBlk, bool kPack>
 __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_move_hist(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
@@ -197,7 +206,7 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_move_hist(Params p) {
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {   // block-uniform trip count
     uint16_t s[kK1Unroll];
     int32_t x[kK1Unroll], y[kK1Unroll], z[kK1Unroll];
-    uint32_t id[kK1Unroll], key[kK1Unroll];
+    uint32_t id[kK1Unroll], key[kK1Unroll], dsp[kK1Unroll];
 #pragma unroll
     for (int a = 0; a < kK1Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
@@ -214,6 +223,7 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_move_hist(Params p) {
       if (s[a] == kDead) continue;
       const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
       key[a] = cell_key(m.x, m.y, m.z, p);
+      if (kPack) dsp[a] = pack_disp(m.x - x[a], m.y - y[a], m.z - z[a], m.s != s[a]);
     }
     uint32_t first[kK1Unroll], rank[kK1Unroll];
     int leader[kK1Unroll];
@@ -227,7 +237,10 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_move_hist(Params p) {
 #pragma unroll
     for (int a = 0; a < kK1Unroll; ++a) {
       const uint32_t f = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]);
-      if (s[a] != kDead) p.off[base + a * kMoveThreads + threadIdx.x] = f + rank[a];
+      if (s[a] != kDead) {
+        p.off[base + a * kMoveThreads + threadIdx.x] = f + rank[a];
+        if (kPack) p.disp[base + a * kMoveThreads + threadIdx.x] = dsp[a];
+      }
     }
   }
 }
@@ -305,18 +318,18 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
 // slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
 // kK3Unroll agents in flight per thread.  Membrane crossings change the species here; their
 // counts deltas go straight to counts row t+1 (rare events).
-template <bool kGaussSmem, int kK3Unroll, int kMinBlk>
+template <bool kGaussSmem, int kK3Unroll, int kMinBlk, bool kPack>
 __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
-  const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
+  const int16_t* g = stage_tables<kGaussSmem && !kPack>(p, M, s_gauss);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
   uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
   constexpr uint32_t kTile = kMoveThreads * kK3Unroll;
   for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {
     uint16_t s[kK3Unroll];
     int32_t x[kK3Unroll], y[kK3Unroll], z[kK3Unroll];
-    uint32_t id[kK3Unroll], off[kK3Unroll];
+    uint32_t id[kK3Unroll], off[kK3Unroll], dsp[kK3Unroll];
 #pragma unroll
     for (int a = 0; a < kK3Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
@@ -327,12 +340,19 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
       if (i < n) {   // not gated on the species: one round trip
         x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; off[a] = p.off[i];
+        if (kPack) dsp[a] = p.disp[i];
       }
     }
 #pragma unroll
     for (int a = 0; a < kK3Unroll; ++a) {
       if (s[a] == kDead) continue;
-      const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
+      Moved m;
+      if (kPack) {
+        m.x = x[a] + unpack10(dsp[a], 0); m.y = y[a] + unpack10(dsp[a], 10); m.z = z[a] + unpack10(dsp[a], 20);
+        m.s = (dsp[a] >> 30 & 1u) ? M.sp[s[a]].cross_to : s[a];
+      } else {
+        m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
+      }
       if (m.s != s[a]) {
         const uint32_t rep = (uint32_t)x[a] >> p.stride_shift;
         atomicSub(&row[rep * p.n_species + s[a]], 1u);

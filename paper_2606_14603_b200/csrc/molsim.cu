@@ -28,7 +28,7 @@ const char* kKernelNames[SIM_N_KERNELS] = {
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t soa[2][5], off, prop, best, hasprop, cell, partial, bits, birth_mid, birth_top, birth_list, counts,
+  size_t soa[2][5], off, disp, prop, best, hasprop, cell, partial, bits, birth_mid, birth_top, birth_list, counts,
       scal, tab, gauss, total;
   uint32_t n_cells, nx, ny, nz;
 };
@@ -43,7 +43,7 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
   const size_t cap = c->capacity;
   for (int b = 0; b < 2; ++b) for (int a = 0; a < 5; ++a) L.soa[b][a] = take(cap * (a < 4 ? 4 : 2) + 64);
-  L.off = take(cap * 4); L.prop = take(cap * 4);
+  L.off = take(cap * 4); L.disp = take(cap * 4); L.prop = take(cap * 4);
   L.best = take(cap * 8);
   L.hasprop = take((cap / 32 + 16) * 4);
   L.cell = take(((size_t)nc + 1 + 1024) * 4);
@@ -150,6 +150,7 @@ struct sim {
   void (*k_move)(Params) = nullptr;   // K1 / K3 instantiation picked at create time (Gaussian tables in shared
   void (*k_scat)(Params) = nullptr;   // memory or not; MoveCfgSmall or MoveCfgLarge)
   uint32_t k1_unroll = 0, k3_unroll = 0;
+  bool pack_disp = false;             // every table entry fits 10 signed bits: K1 hands the displacement to K3
   size_t gauss_bytes = 0;
   uint32_t grid_move = 0, grid_scatter = 0, grid_pairs = 0, grid_uni = 0, grid_resolve = 0;
   uint32_t cell_seg = 0, scan_blocks = 1, tail_blocks = 1;
@@ -228,7 +229,8 @@ int enqueue_step(sim* s) {
     k_cell_reduce<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_CELL_SCAN);
     k_cell_scan<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
-  { ProfScope ps(s, KI_SCATTER); s->k_scat<<<s->grid_scatter, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_SCATTER);
+    s->k_scat<<<s->grid_scatter, kMoveThreads, (s->gauss_in_smem && !s->pack_disp) ? s->gauss_bytes : 0, s->run>>>(p); }
   { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
@@ -284,6 +286,14 @@ void build_graphs(sim* s) {
   s->graphs_ok = ok;
 }
 
+}  // namespace
+
+namespace {
+template <bool kGauss, bool kPack> void pick_move_kernels(sim* s, bool large) {
+  using S_ = MoveCfgSmall; using L_ = MoveCfgLarge;
+  s->k_move = large ? k_move_hist<kGauss, L_::k1u, L_::k1b, kPack> : k_move_hist<kGauss, S_::k1u, S_::k1b, kPack>;
+  s->k_scat = large ? k_scatter<kGauss, L_::k3u, L_::k3b, kPack> : k_scatter<kGauss, S_::k3u, S_::k3b, kPack>;
+}
 }  // namespace
 
 extern "C" {
@@ -354,7 +364,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
                                      (int32_t*)(w + L.soa[b][2]), (uint32_t*)(w + L.soa[b][3]),
                                      (uint16_t*)(w + L.soa[b][4])}; };
   p.cur = soa(0); p.oth = soa(1);
-  p.off = (uint32_t*)(w + L.off); p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
+  p.off = (uint32_t*)(w + L.off); p.disp = (uint32_t*)(w + L.disp); p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
   p.best = (unsigned long long*)(w + L.best);
   p.cell = (uint32_t*)(w + L.cell); p.partial = (uint32_t*)(w + L.partial);
   p.bits = (uint32_t*)(w + L.bits); p.birth_mid = (uint32_t*)(w + L.birth_mid); p.birth_top = (uint32_t*)(w + L.birth_top);
@@ -386,6 +396,14 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
 
   s->gauss_bytes = ((size_t)cfg->n_sigma_classes << cfg->table_bits) * 2;
   s->gauss_in_smem = s->gauss_bytes <= 160 * 1024;
+  {
+    int32_t max_tab = 0;
+    for (size_t i = 0; i < ((size_t)cfg->n_sigma_classes << cfg->table_bits); ++i)
+      max_tab = std::max<int32_t>(max_tab, std::abs((int32_t)cfg->tables[i]));
+    // measured: the extra 4 B/agent stream pays while the state is L2-resident (W3 -6 %, W4 1M -3.5 %) and
+    // costs 10 % at 16 M agents, where K1/K3 are sensitive to every additional HBM stream
+    s->pack_disp = max_tab <= 511 && cfg->capacity < kLargeFrom;
+  }
   // persistent grids: resident blocks per SM (occupancy API) x SM count, capped by the work there is
   {
     int dev = 0, sms = 148;
@@ -399,13 +417,8 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     const size_t gsm = s->gauss_in_smem ? s->gauss_bytes : 0;
     using S_ = MoveCfgSmall; using L_ = MoveCfgLarge;
     const bool large = cfg->capacity >= kLargeFrom;
-    if (gsm) {
-      s->k_move = large ? k_move_hist<true, L_::k1u, L_::k1b> : k_move_hist<true, S_::k1u, S_::k1b>;
-      s->k_scat = large ? k_scatter<true, L_::k3u, L_::k3b> : k_scatter<true, S_::k3u, S_::k3b>;
-    } else {
-      s->k_move = large ? k_move_hist<false, L_::k1u, L_::k1b> : k_move_hist<false, S_::k1u, S_::k1b>;
-      s->k_scat = large ? k_scatter<false, L_::k3u, L_::k3b> : k_scatter<false, S_::k3u, S_::k3b>;
-    }
+    if (gsm) { if (s->pack_disp) pick_move_kernels<true, true>(s, large); else pick_move_kernels<true, false>(s, large); }
+    else { if (s->pack_disp) pick_move_kernels<false, true>(s, large); else pick_move_kernels<false, false>(s, large); }
     s->k1_unroll = large ? L_::k1u : S_::k1u; s->k3_unroll = large ? L_::k3u : S_::k3u;
     if (gsm > 48 * 1024) {
       cudaFuncSetAttribute(s->k_move, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
@@ -414,7 +427,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_move, kMoveThreads, gsm);
     s->grid_move = sized(occ, (uint64_t)kMoveThreads * s->k1_unroll);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_scat, kMoveThreads, gsm);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_scat, kMoveThreads, s->pack_disp ? 0 : gsm);
     s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * s->k3_unroll);
     s->grid_pairs = (uint32_t)(((uint64_t)cfg->capacity + kPairThreads - 1) / kPairThreads);   // one tile per block
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, kUniThreads, 0);
