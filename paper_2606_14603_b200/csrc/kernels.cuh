@@ -443,7 +443,7 @@ struct PairWarpSmem {                   // private to one warp
   uint32_t hit_j[kWarpHitCap];          // candidate slot that passed the window test
   uint8_t hit_o[kWarpHitCap];           // owner thread
   uint16_t task[kWarpTaskCap];          // owner thread | row code (5..8) << 8
-  uint32_t nhit;
+  uint32_t nhit, ntask;
 };
 struct PairSmem {
   int4 pos[kPairThreads];               // x, y, z, species | forward-row mask << 16
@@ -529,7 +529,7 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, tid = threadIdx.x;
   PairWarpSmem& W = S.w[warp];
   const int32_t R = p.max_r, cs = p.cell_size;
-  if (lane == 0) W.nhit = 0;
+  if (lane == 0) { W.nhit = 0; W.ntask = 0; }
   const uint32_t i = base + tid;
   uint32_t s = kDead;
   int32_t x = 0, y = 0, z = 0;
@@ -559,15 +559,15 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
     if (j1 > base + kPairThreads) scan_global(p, W, base + kPairThreads, j1, tid, x, y, z);
   }
 
-  // ---- B: the warp's task list: one ballot per forward row code
-  uint32_t nt = 0;
-#pragma unroll
-  for (uint32_t c = 5u; c <= 8u; ++c) {
-    const uint32_t m = __ballot_sync(0xFFFFFFFFu, (need >> c) & 1u);
-    if ((need >> c) & 1u) W.task[nt + __popc(m & ((1u << lane) - 1u))] = (uint16_t)(tid | (c << 8));
-    nt += __popc(m);
+  // ---- B: the warp's task list: the ~20 % of lanes that face a +y / +z cell append their forward rows
+  // (order is irrelevant: every hit is merged by atomicMin)
+  if (need >> 5) {
+    uint32_t m = need >> 5;
+    uint32_t pos = atomicAdd(&W.ntask, (uint32_t)__popc(m));
+    for (; m; m &= m - 1u) W.task[pos++] = (uint16_t)(tid | ((uint32_t)(__ffs(m) + 4) << 8));
   }
   __syncwarp();
+  const uint32_t nt = W.ntask;
 
   // ---- C: the forward rows: 4, 2 or 1 lanes per task
   {
