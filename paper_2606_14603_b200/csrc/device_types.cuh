@@ -56,9 +56,14 @@ struct Scalars {
   uint32_t t_first[kMaxRules];
 };
 
-// One agent array set (structure of arrays, north_star (1)).
+// One agent array set (north_star (1): int32 fixed-point x, y, z, uint32 id, uint16 species = 18 B/agent, all
+// integer).  Two parallel arrays: a 16-byte record {x, y, z, id} and the species.  Round 1 kept five separate
+// arrays; K1 and K3 turned out to be bound by the NUMBER of HBM streams they keep open, so
+// the four 32-bit fields that always travel together are read with one 128-bit load and written with one
+// 128-bit store.  The C ABI still speaks separate arrays.
 struct Soa {
-  int32_t* x; int32_t* y; int32_t* z; uint32_t* id; uint16_t* sp;
+  int4* r;          // {x, y, z, (int32) id}
+  uint16_t* sp;
 };
 
 struct Params {

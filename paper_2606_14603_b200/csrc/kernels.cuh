@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_move_hist(Params p) {
 #pragma unroll
     for (int a = 0; a < kK1Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
-      if (i < n) { x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; }   // not gated on the species: one round trip
+      if (i < n) { const int4 q = p.cur.r[i]; x[a] = q.x; y[a] = q.y; z[a] = q.z; id[a] = (uint32_t)q.w; }   // one 128-bit load, not gated on the species
     }
 #pragma unroll
     for (int a = 0; a < kK1Unroll; ++a) {
@@ -255,8 +255,9 @@ __global__ void __launch_bounds__(kMoveThreads) k_move_only(Params p) {
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const uint16_t s = p.cur.sp[i];
     if (s == kDead) continue;
-    const Moved m = move_agent(p, M, g, s, p.cur.x[i], p.cur.y[i], p.cur.z[i], p.cur.id[i], t);
-    p.cur.x[i] = m.x; p.cur.y[i] = m.y; p.cur.z[i] = m.z; p.cur.sp[i] = m.s;
+    const int4 q = p.cur.r[i];
+    const Moved m = move_agent(p, M, g, s, q.x, q.y, q.z, (uint32_t)q.w, t);
+    p.cur.r[i] = make_int4(m.x, m.y, m.z, q.w); p.cur.sp[i] = m.s;
   }
 }
 
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
     for (int a = 0; a < kK3Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
       if (i < n) {   // not gated on the species: one round trip
-        x[a] = p.cur.x[i]; y[a] = p.cur.y[i]; z[a] = p.cur.z[i]; id[a] = p.cur.id[i]; off[a] = p.off[i];
+        const int4 q = p.cur.r[i]; x[a] = q.x; y[a] = q.y; z[a] = q.z; id[a] = (uint32_t)q.w; off[a] = p.off[i];
         if (kPack) dsp[a] = p.disp[i];
       }
     }
@@ -365,8 +366,7 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
     for (int a = 0; a < kK3Unroll; ++a) {
       if (s[a] == kDead) continue;
       const uint32_t dst = off[a];
-      p.oth.x[dst] = x[a]; p.oth.y[dst] = y[a]; p.oth.z[dst] = z[a];
-      p.oth.id[dst] = id[a];
+      p.oth.r[dst] = make_int4(x[a], y[a], z[a], (int32_t)id[a]);     // ONE scattered 128-bit store per agent
       p.oth.sp[dst] = s[a];
     }
   }
@@ -427,7 +427,7 @@ __device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t
   if (e == 0xFFu) return;
   const DevRx& rx = T->rx[e];
   if (d2 > rx.r2) return;
-  const uint32_t id = p.oth.id[i], idj = p.oth.id[j];
+  const uint32_t id = (uint32_t)p.oth.r[i].w, idj = (uint32_t)p.oth.r[j].w;
   const uint4 r = philox_sim(p, min(id, idj), max(id, idj), t, kTagPair);
   if (!fire(r.x, rx.thr)) return;
   const unsigned long long hi = (unsigned long long)d2 << 32, ki = hi | idj, kj = hi | id;
@@ -476,12 +476,11 @@ __device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, ui
   const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
   const int32_t ox = R - x, oy = R - y, oz = R - z;
-  const int32_t* __restrict__ X = p.oth.x;
-  const int32_t* __restrict__ Y = p.oth.y;
-  const int32_t* __restrict__ Z = p.oth.z;
+  const int4* __restrict__ Rr = p.oth.r;
 #pragma unroll 2
   for (uint32_t j = j0; j < j1; ++j) {
-    const uint32_t ux = (uint32_t)(__ldg(X + j) + ox), uy = (uint32_t)(__ldg(Y + j) + oy), uz = (uint32_t)(__ldg(Z + j) + oz);
+    const int4 q = __ldg(Rr + j);
+    const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
     if (max(max(ux, uy), uz) <= R2) push_hit(W, owner, j);
   }
 }
@@ -510,7 +509,8 @@ __device__ __noinline__ void slow_agent(const Params* pp, const PairSmem* Sp, ui
     const uint32_t r2 = row_of(p, rowc, c);
     const uint32_t j0 = c == 4u ? i + 1u : p.cell[r2 + xlo], j1 = p.cell[r2 + xlo + nxr + 1];
     for (uint32_t j = j0; j < j1; ++j) {
-      const long long dx = (long long)p.oth.x[j] - x, dy = (long long)p.oth.y[j] - y, dz = (long long)p.oth.z[j] - z;
+      const int4 qj = p.oth.r[j];
+      const long long dx = (long long)qj.x - x, dy = (long long)qj.y - y, dz = (long long)qj.z - z;
       if (dx > R || dx < -R || dy > R || dy < -R || dz > R || dz < -R) continue;
       const unsigned long long d2 = (unsigned long long)(dx * dx + dy * dy + dz * dz);
       if (d2 <= p.max_r2) pair_merge(p, i, j, (uint32_t)d2, si, t);
@@ -533,7 +533,7 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
   const uint32_t i = base + tid;
   uint32_t s = kDead;
   int32_t x = 0, y = 0, z = 0;
-  if (i < n) { s = p.oth.sp[i]; x = p.oth.x[i]; y = p.oth.y[i]; z = p.oth.z[i]; }
+  if (i < n) { s = p.oth.sp[i]; const int4 q = p.oth.r[i]; x = q.x; y = q.y; z = q.z; }
   const bool active = s != kDead && ((p.binds_mask >> s) & 1ull);
   uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0, j1 = 0;
   if (active) {
@@ -589,7 +589,8 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
     for (uint32_t h = lane; h < nh; h += 32u) {
       const uint32_t owner = W.hit_o[h], j = W.hit_j[h];
       const int4 q = S.pos[owner];
-      const int32_t dx = p.oth.x[j] - q.x, dy = p.oth.y[j] - q.y, dz = p.oth.z[j] - q.z;   // each within +-R
+      const int4 qj = p.oth.r[j];
+      const int32_t dx = qj.x - q.x, dy = qj.y - q.y, dz = qj.z - q.z;   // each within +-R
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
       if (d2 <= p.max_r2) pair_merge(p, base + owner, j, d2, (uint32_t)q.w & 0xFFFFu, t);
     }
@@ -608,7 +609,8 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
 // neighbourhood sweep, used only when bslot[i] lost a store race (see K4, D).
 __device__ __noinline__ uint32_t find_partner(const Params* pp, uint32_t i, uint32_t idj) {
   const Params& p = *pp;
-  const int32_t x = p.oth.x[i], y = p.oth.y[i], z = p.oth.z[i], R = p.max_r;
+  const int4 qi = p.oth.r[i];
+  const int32_t x = qi.x, y = qi.y, z = qi.z, R = p.max_r;
   const int32_t xlo = cell_coord(max(x - R, 0), p), xhi = min(cell_coord(x + R, p), p.nx - 1);
   const int32_t ylo = cell_coord(max(y - R, 0), p), yhi = min(cell_coord(y + R, p), p.ny - 1);
   const int32_t zlo = cell_coord(max(z - R, 0), p), zhi = min(cell_coord(z + R, p), p.nz - 1);
@@ -616,7 +618,7 @@ __device__ __noinline__ uint32_t find_partner(const Params* pp, uint32_t i, uint
     for (int32_t cy = ylo; cy <= yhi; ++cy) {
       const uint32_t rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
       for (uint32_t j = p.cell[rowc + xlo]; j < p.cell[rowc + xhi + 1]; ++j)
-        if (p.oth.id[j] == idj) return j;
+        if ((uint32_t)p.oth.r[j].w == idj) return j;
     }
   return kNoProp;
 }
@@ -635,16 +637,16 @@ __global__ void __launch_bounds__(256) k_resolve(const __grid_constant__ Params 
       const uint32_t i = w * 32u + b;
       const uint32_t idj = (uint32_t)p.best[i];            // low word of (d2, id of the proposed partner)
       uint32_t j = p.prop[i];
-      if (j >= n || p.oth.id[j] != idj) j = find_partner(&p, i, idj);
+      if (j >= n || (uint32_t)p.oth.r[j].w != idj) j = find_partner(&p, i, idj);
       if (j <= i || j >= n) continue;                         // the lower slot handles the pair
-      const uint32_t idi = p.oth.id[i];
+      const uint32_t idi = (uint32_t)p.oth.r[i].w;
       if ((uint32_t)p.best[j] != idi) continue;               // not mutual (best[j] = kNoKey if j never proposed)
       const uint16_t si = p.oth.sp[i], sj = p.oth.sp[j];
       const DevRx& rx = T->rx[T->rxmap[(uint32_t)si * kMaxSpecies + sj]];
       const bool anchor_i = (si != sj) ? (si == rx.a) : (idi < idj);
       p.oth.sp[i] = anchor_i ? rx.cplx : kDead;
       p.oth.sp[j] = anchor_i ? kDead : rx.cplx;
-      int32_t* d = s_delta + ((uint32_t)p.oth.x[i] >> p.stride_shift) * p.n_species;
+      int32_t* d = s_delta + ((uint32_t)p.oth.r[i].x >> p.stride_shift) * p.n_species;
       atomicSub(&d[si], 1); atomicSub(&d[sj], 1); atomicAdd(&d[rx.cplx], 1);
     }
   }
@@ -662,7 +664,7 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
                                         uint32_t t, int32_t* s_delta) {
   const DevSpecies& S = T->sp[s0];
   const uint32_t nch = S.n_channels;
-  const uint32_t id = p.oth.id[i];
+  const uint32_t id = (uint32_t)p.oth.r[i].w;
   const uint4 r = philox_sim(p, id, 0u, t, kTagUni);
   const uint32_t rr[4] = {r.x, r.y, r.z, r.w};
   bool consumed = false;
@@ -693,7 +695,7 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
     }
   }
   if (s == s0 && !mask) return;
-  int32_t* d = s_delta + ((uint32_t)p.oth.x[i] >> p.stride_shift) * p.n_species;
+  int32_t* d = s_delta + ((uint32_t)p.oth.r[i].x >> p.stride_shift) * p.n_species;
   if (s != s0) {
     p.oth.sp[i] = s;
     atomicSub(&d[s0], 1);
@@ -821,7 +823,7 @@ __global__ void __launch_bounds__(kScanThreads) k_births(Params p) {
   for (uint32_t e = blockIdx.x * wpb + (threadIdx.x >> 5); e < nb; e += gridDim.x * wpb) {
     const uint2 ent = p.birth_list[e];
     const uint32_t slot = ent.x, mask = ent.y & 0xFu, pre = ent.y >> 16;
-    const uint32_t pid = p.oth.id[slot];
+    const uint32_t pid = (uint32_t)p.oth.r[slot].w;
     uint32_t part = 0;
     for (uint32_t j = ((pid >> p.top_shift) << (p.top_shift - kMidShift)) + lane; j < (pid >> kMidShift); j += 32u)
       part += p.birth_mid[j];
@@ -831,7 +833,8 @@ __global__ void __launch_bounds__(kScanThreads) k_births(Params p) {
     const uint32_t rank0 = s_top[pid >> p.top_shift] + __reduce_add_sync(0xFFFFFFFFu, part);
     if (lane < 4u && (mask >> lane & 1u)) {
       const uint32_t k = lane, rank = rank0 + __popc(mask & ((1u << k) - 1u));
-      const int32_t px = p.oth.x[slot], py = p.oth.y[slot], pz = p.oth.z[slot];
+      const int4 qp = p.oth.r[slot];
+      const int32_t px = qp.x, py = qp.y, pz = qp.z;
       const int32_t rbase = (int32_t)(((uint32_t)px >> p.stride_shift) << p.stride_shift);
       const int32_t lx = px - rbase;
       const uint16_t sp_new = T->sp[pre].ch[k].prod1;
@@ -843,8 +846,7 @@ __global__ void __launch_bounds__(kScanThreads) k_births(Params p) {
       if (c.shape == 0) { qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L); }
       else if (!comp_valid(c, qx, qy, qz)) { qx = lx; qy = py; qz = pz; }
       const uint32_t dst = n_sorted + rank;
-      p.oth.x[dst] = qx + rbase; p.oth.y[dst] = qy; p.oth.z[dst] = qz;
-      p.oth.id[dst] = next_id + rank;
+      p.oth.r[dst] = make_int4(qx + rbase, qy, qz, (int32_t)(next_id + rank));
       p.oth.sp[dst] = sp_new;
     }
   }
@@ -858,7 +860,7 @@ __global__ void __launch_bounds__(256) k_epilogue(Params p) {
   const uint32_t nb = p.scal->birth_count;
   const uint32_t stride = gridDim.x * blockDim.x;
   for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < nb; e += stride) {
-    const uint32_t pid = p.oth.id[p.birth_list[e].x];
+    const uint32_t pid = (uint32_t)p.oth.r[p.birth_list[e].x].w;
     p.bits[pid >> 3] = 0u; p.birth_mid[pid >> kMidShift] = 0u; p.birth_top[pid >> p.top_shift] = 0u;
   }
   __threadfence();
@@ -905,7 +907,7 @@ __global__ void k_seed(Params p, uint32_t species, uint32_t replica, uint32_t co
       }
     }
     const uint32_t d = dst_base + n;
-    p.cur.x[d] = x + rbase; p.cur.y[d] = y; p.cur.z[d] = z; p.cur.id[d] = id;
+    p.cur.r[d] = make_int4(x + rbase, y, z, (int32_t)id);
     p.cur.sp[d] = (uint16_t)species;
   }
 }
@@ -919,9 +921,10 @@ __global__ void __launch_bounds__(256) k_count_row(Params p, uint32_t r, uint32_
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += gridDim.x * blockDim.x) {
     const uint16_t s = p.cur.sp[i];
     if (s == kDead) continue;
-    const uint32_t rep = (uint32_t)p.cur.x[i] >> p.stride_shift;
+    const int4 q = p.cur.r[i];
+    const uint32_t rep = (uint32_t)q.x >> p.stride_shift;
     // sim_load_agents hands us caller data: species, replica tile and id are validated here (err bit 2)
-    if (s >= p.n_species || rep >= p.n_replicas || p.cur.id[i] >= next_id) { atomicOr(&p.scal->err, 4u); continue; }
+    if (s >= p.n_species || rep >= p.n_replicas || (uint32_t)q.w >= next_id) { atomicOr(&p.scal->err, 4u); continue; }
     atomicAdd(&s_delta[rep * p.n_species + s], 1);
   }
   delta_flush(s_delta, p.counts + (size_t)r * p.row_width, p.row_width);
@@ -932,7 +935,7 @@ __global__ void k_copy_row(Params p, uint32_t r) {
   for (uint32_t k = threadIdx.x; k < p.row_width; k += blockDim.x) dst[k] = src[k];
 }
 
-// sim_read_agents: gather live agents into the scratch (oth) arrays (warp-aggregated append).
+// sim_read_agents: gather live agents into the scratch (oth) buffers (warp-aggregated append).
 __global__ void __launch_bounds__(256) k_gather_live(Params p, uint32_t n_slots) {
   const uint32_t lane = threadIdx.x & 31u;
   for (uint32_t base = blockIdx.x * blockDim.x; base < n_slots; base += gridDim.x * blockDim.x) {
@@ -943,9 +946,21 @@ __global__ void __launch_bounds__(256) k_gather_live(Params p, uint32_t n_slots)
     if (lane == 0 && live) d = atomicAdd(&p.scal->n_read, (uint32_t)__popc(live));
     d = __shfl_sync(0xFFFFFFFFu, d, 0) + __popc(live & ((1u << lane) - 1u));
     if (s == kDead) continue;
-    p.oth.x[d] = p.cur.x[i]; p.oth.y[d] = p.cur.y[i]; p.oth.z[d] = p.cur.z[i];
-    p.oth.id[d] = p.cur.id[i]; p.oth.sp[d] = s;
+    // the C ABI speaks separate arrays: the scratch record buffer is written as four planes of `capacity` words
+    const int4 q = p.cur.r[i];
+    int32_t* plane = reinterpret_cast<int32_t*>(p.oth.r);
+    plane[d] = q.x; plane[(size_t)p.capacity + d] = q.y; plane[2 * (size_t)p.capacity + d] = q.z;
+    plane[3 * (size_t)p.capacity + d] = q.w; p.oth.sp[d] = s;
   }
+}
+
+// sim_load_agents: the caller's separate x / y / z / id arrays were copied into the four planes of the scratch
+// record buffer; interleave them into the current records.
+__global__ void __launch_bounds__(256) k_pack_records(Params p, uint32_t n) {
+  const int32_t* plane = reinterpret_cast<const int32_t*>(p.oth.r);
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    p.cur.r[i] = make_int4(plane[i], plane[(size_t)p.capacity + i], plane[2 * (size_t)p.capacity + i],
+                           plane[3 * (size_t)p.capacity + i]);
 }
 
 }  // namespace molsim

@@ -28,7 +28,7 @@ const char* kKernelNames[SIM_N_KERNELS] = {
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t soa[2][5], off, disp, prop, best, hasprop, cell, partial, bits, birth_mid, birth_top, birth_list, counts,
+  size_t soa[2][2], off, disp, prop, best, hasprop, cell, partial, bits, birth_mid, birth_top, birth_list, counts,
       scal, tab, gauss, total;
   uint32_t n_cells, nx, ny, nz;
 };
@@ -42,7 +42,7 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
   const size_t cap = c->capacity;
-  for (int b = 0; b < 2; ++b) for (int a = 0; a < 5; ++a) L.soa[b][a] = take(cap * (a < 4 ? 4 : 2) + 64);
+  for (int b = 0; b < 2; ++b) { L.soa[b][0] = take(cap * 16 + 64); L.soa[b][1] = take(cap * 2 + 64); }   // records, species
   L.off = take(cap * 4); L.disp = take(cap * 4); L.prop = take(cap * 4);
   L.best = take(cap * 8);
   L.hasprop = take((cap / 32 + 16) * 4);
@@ -248,7 +248,7 @@ namespace {
 
 constexpr uint32_t kGraphSteps = 8;   // even, so the parity after the graph equals the parity before
 
-int parity_of(const sim* s) { return s->prm.cur.x == (const int32_t*)(s->ws + s->lay.soa[0][0]) ? 0 : 1; }
+int parity_of(const sim* s) { return s->prm.cur.r == (const int4*)(s->ws + s->lay.soa[0][0]) ? 0 : 1; }
 
 // Captures `steps` steps starting at the current parity into an executable graph; the handle's
 // host-side state is restored afterwards (capturing executes nothing).
@@ -360,9 +360,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   Params& p = s->prm;
   std::memset(&p, 0, sizeof(p));
   char* w = s->ws;
-  auto soa = [&](int b) { return Soa{(int32_t*)(w + L.soa[b][0]), (int32_t*)(w + L.soa[b][1]),
-                                     (int32_t*)(w + L.soa[b][2]), (uint32_t*)(w + L.soa[b][3]),
-                                     (uint16_t*)(w + L.soa[b][4])}; };
+  auto soa = [&](int b) { return Soa{(int4*)(w + L.soa[b][0]), (uint16_t*)(w + L.soa[b][1])}; };
   p.cur = soa(0); p.oth = soa(1);
   p.off = (uint32_t*)(w + L.off); p.disp = (uint32_t*)(w + L.disp); p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
   p.best = (unsigned long long*)(w + L.best);
@@ -581,7 +579,9 @@ int sim_read_agents(sim_t* s, uint32_t cap, int32_t* x, int32_t* y, int32_t* z, 
   if (n > cap) return SIM_E_CAPACITY;
   if (n == 0) return SIM_OK;
   std::vector<uint32_t> hid(n);
-  CK(cudaMemcpy(hid.data(), s->prm.oth.id, (size_t)n * 4, cudaMemcpyDeviceToHost));
+  const int32_t* plane = reinterpret_cast<const int32_t*>(s->prm.oth.r);   // k_gather_live wrote four planes
+  const size_t pstride = s->cfg.capacity;
+  CK(cudaMemcpy(hid.data(), plane + 3 * pstride, (size_t)n * 4, cudaMemcpyDeviceToHost));
   // id-sorted order: ids are unique and < next_id, so one pass over the id space sorts them
   std::vector<uint32_t> where((size_t)sc.next_id, 0xFFFFFFFFu), order;
   order.reserve(n);
@@ -589,7 +589,7 @@ int sim_read_agents(sim_t* s, uint32_t cap, int32_t* x, int32_t* y, int32_t* z, 
   for (uint32_t v = 0; v < sc.next_id; ++v) if (where[v] != 0xFFFFFFFFu) order.push_back(where[v]);
   if (order.size() != n) return SIM_E_INVAL;   // duplicate ids: internal error
   std::vector<int32_t> tmp(n);
-  const int32_t* srcs[3] = {s->prm.oth.x, s->prm.oth.y, s->prm.oth.z};
+  const int32_t* srcs[3] = {plane, plane + pstride, plane + 2 * pstride};
   int32_t* dsts[3] = {x, y, z};
   for (int a = 0; a < 3; ++a) {
     if (!dsts[a]) continue;
@@ -613,10 +613,18 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
   Scalars sc;
   int r = read_scalars(s, &sc);
   if (r) return r;
-  CK(cudaMemcpyAsync(s->prm.cur.x, x, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->prm.cur.y, y, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->prm.cur.z, z, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->prm.cur.id, id, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+  {
+    int32_t* plane = reinterpret_cast<int32_t*>(s->prm.oth.r);   // scratch: four planes, then k_pack_records
+    const size_t pstride = s->cfg.capacity;
+    CK(cudaMemcpyAsync(plane, x, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+    CK(cudaMemcpyAsync(plane + pstride, y, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+    CK(cudaMemcpyAsync(plane + 2 * pstride, z, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+    CK(cudaMemcpyAsync(plane + 3 * pstride, id, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+    if (n) {
+      ProfScope ps(s, KI_OTHER);
+      k_pack_records<<<std::min<uint32_t>((n + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, n);
+    }
+  }
   CK(cudaMemcpyAsync(s->prm.cur.sp, species, (size_t)n * 2, cudaMemcpyHostToDevice, s->stream));
   sc.n_slots = n; sc.next_id = next_id; sc.t = step; sc.err = 0;
   sc.birth_count = sc.total_births = sc.ticket = 0;

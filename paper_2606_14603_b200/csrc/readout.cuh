@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(kMonThreads) k_monitor(const uint32_t* __restr
 
 // ----------------------------------------------------------------------------- N4 headless picture
 // Pass 1: every live agent of the replica inside the window adds one to the counter of its
-// (pixel, compartment) — a streaming read of x, y, z, species with warp-level runs of equal pixels merged
+// (pixel, compartment) — a streaming read of the records and species with warp-level runs of equal pixels merged
 // before the atomic (agents are cell-sorted, so neighbours in memory are neighbours in space).
 // Pass 2: one thread per pixel turns the counters into RGBA (reading S25).
 struct DevView {
@@ -80,9 +80,10 @@ __global__ void __launch_bounds__(256) k_splat_count(Params p, DevView v, uint32
     uint32_t key = 0xFFFFFFFFu;
     if (i < n_slots) {
       const uint16_t s = p.cur.sp[i];
-      const int32_t x = p.cur.x[i];
+      const int4 r = p.cur.r[i];
+      const int32_t x = r.x;
       if (s != kDead && ((uint32_t)x >> p.stride_shift) == v.replica) {
-        const int32_t q[3] = {x - (int32_t)(v.replica << p.stride_shift), p.cur.y[i], p.cur.z[i]};
+        const int32_t q[3] = {x - (int32_t)(v.replica << p.stride_shift), r.y, r.z};
         const int32_t u = v.axis == 0 ? q[1] : q[0], w = v.axis == 2 ? q[1] : q[2];
         const long long du = (long long)u - v.u0, dv = (long long)w - v.v0;
         if (du >= 0 && du < (long long)v.eu && dv >= 0 && dv < (long long)v.ev) {
