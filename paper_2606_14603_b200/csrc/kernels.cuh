@@ -179,10 +179,16 @@ __device__ __forceinline__ void run_of_key(uint32_t key, uint32_t lane, int& lea
 }
 
 // Agents in flight per thread (kU) and resident blocks per SM (kB) are template parameters of K1 and
-// K3; the host picks per problem size (swept on B200: profiles/r1d_kernels.md).  Many thin blocks
-// finish a small population sooner; fewer, fatter blocks win from a few million agents on.
+// K3; the host picks per problem size (swept on B200: profiles/r1e_kernels.md).  With the 16-byte records
+// K1 likes 4 agents per thread x 4 blocks/SM from a few million agents on; K3 keeps 2 x 5 at every size.
 struct MoveCfgSmall { static constexpr int k1u = 2, k1b = 5, k3u = 2, k3b = 5; };
-struct MoveCfgLarge { static constexpr int k1u = 4, k1b = 3, k3u = 3, k3b = 3; };
+#ifndef MOLSIM_L_K1U      // tuning builds override the large-population shape
+#define MOLSIM_L_K1U 4
+#define MOLSIM_L_K1B 4
+#define MOLSIM_L_K3U 2
+#define MOLSIM_L_K3B 5
+#endif
+struct MoveCfgLarge { static constexpr int k1u = MOLSIM_L_K1U, k1b = MOLSIM_L_K1B, k3u = MOLSIM_L_K3U, k3b = MOLSIM_L_K3B; };
 constexpr uint32_t kLargeFrom = 2000000;   // capacity (agents) from which MoveCfgLarge is used
 constexpr int kMoveThreads = 256;
 
