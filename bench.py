@@ -135,7 +135,7 @@ def moved_bytes_per_agent(kernel, c):
         "k_move_hist": 18 + 4 + 8 * c,           # R soa, W off, cell count RMW (moved positions are not stored)
         "memset_cells": 4 * c, "k_cell_reduce": 4 * c, "k_cell_scan": 8 * c,
         "k_scatter": 18 + 4 + 18 + 4 * c,        # R soa + off, W soa, R cell starts
-        "k_pairs": 14 + 0.125 + 4 * c,           # R xyz + species, W 1 bit; R cell starts
+        "k_pairs": 18 + 0.125 + 4 * c,           # R record + species, W 1 bit; R cell starts
         "k_resolve": 0.125,                      # R proposal bitmap
         "k_uni": 2,                              # R species (id / position only where a channel exists)
     }.get(kernel, 0.0)

@@ -92,6 +92,7 @@ struct Params {
   int32_t cell_size;
   uint32_t cell_magic, cell_mshift;   // v / cell_size == umulhi(v, cell_magic) >> cell_mshift for 0 <= v < 2^31
   int32_t nx, ny, nz;
+  int32_t fwd_row[4];       // cell-index offset of the forward rows (y+1, z), (y-1, z+1), (y, z+1), (y+1, z+1)
   uint32_t n_cells;
   int32_t max_r;            // max interaction radius (ceil sqrt of max r2)
   uint32_t max_r2;

@@ -581,7 +581,7 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
     for (uint32_t k = lane; k < items; k += 32u) {
       const uint32_t e = W.task[k >> lg], owner = e & 0xFFu, part = k & ((1u << lg) - 1u);
       const uint32_t xr = S.xr[owner], oxlo = xr & 0x3FFFFFFFu, onx = xr >> 30;
-      const uint32_t r2 = row_of(p, S.row[owner], e >> 8);
+      const uint32_t r2 = S.row[owner] + (uint32_t)p.fwd_row[(e >> 8) - 5u];   // host-precomputed row offsets of codes 5..8
       const int4 q = S.pos[owner];
       const uint32_t j0 = p.cell[r2 + oxlo], len = p.cell[r2 + oxlo + onx + 1] - j0;
       scan_global(p, W, j0 + ((len * part) >> lg), j0 + ((len * (part + 1u)) >> lg), owner, q.x, q.y, q.z);

@@ -385,6 +385,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     if (T.sp[i].n_channels) p.chan_mask |= 1ull << i;
   }
   p.nx = (int32_t)L.nx; p.ny = (int32_t)L.ny; p.nz = (int32_t)L.nz; p.n_cells = L.n_cells;
+  p.fwd_row[0] = p.nx; p.fwd_row[1] = (p.ny - 1) * p.nx; p.fwd_row[2] = p.ny * p.nx; p.fwd_row[3] = (p.ny + 1) * p.nx;
   p.max_r2 = max_r2;
   p.max_r = (int32_t)std::ceil(std::sqrt((double)max_r2));
   while ((uint64_t)p.max_r * p.max_r < max_r2) p.max_r++;
