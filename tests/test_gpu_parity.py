@@ -237,6 +237,19 @@ def test_large_capacity_kernel_configuration(gpu):
     run_both(gpu, m, 60, chunks=2)
 
 
+def test_crowded_single_cell(gpu):
+    """70,000 non-binding agents in ONE cell (ranks far beyond 16 bits, one histogram counter taking every
+    atomic); a second pair of species keeps a few bindings going in the same cell."""
+    X, A, B, Cx = 0, 1, 2, 3
+    m = Model(name="crowded", species=[Species("X", 1), Species("A", 1), Species("B", 1), Species("C", 2)],
+              reactions=[Reaction(A, B, Cx, 2500, prob_to_thr(0.5))],
+              compartments=[Compartment(SHAPE_CUBE, L=3000)], table_bits=12,
+              tables=stack_tables([44.7214, 31.6228], 12), extent=(3000,) * 3, seed=5, place_seed=6,
+              seed_records=[SeedRecord(X, 70_000), SeedRecord(A, 300), SeedRecord(B, 300)], n_steps=3, cell_size=4096)
+    m.finalize()
+    run_both(gpu, m, 3, chunks=1)
+
+
 def test_w4_1m_full_size_steps(gpu):
     """[CFG 4] N = 1 M in the bench launch configuration, 6 steps, full state compare."""
     m = configs.w4(n=1_000_000, n_steps=6)
