@@ -127,3 +127,20 @@ def test_picture_parity_replicas_and_dense_cube(gpu):
         sim.render(width=4096, height=4096)            # more pixels than the scratch of a 10 k-agent handle
     with pytest.raises(gpu.SimError):
         sim.render(axis=3)
+
+
+def test_compiled_physical_model_parity(gpu):
+    """N2: a model given in physical units (molecular weights, concentrations, k_cat, volume) is compiled to
+    integer tables by workloads/compiler.py and stepped on both sides: bit-exact state and counts."""
+    from oracle.binding import Oracle
+    from test_model_compiler import toy
+    from workloads import compiler
+
+    m = compiler.compile_model(toy(), cell_size=64)
+    sim, orc = gpu.Sim(m), Oracle(m)
+    for s in (sim, orc):
+        s.seed_population(); s.step(50)
+    a, b = sim.read_agents(), orc.read_agents()
+    for k in ("id", "species", "x", "y", "z"):
+        assert np.array_equal(a[k], b[k]), k
+    assert np.array_equal(sim.read_counts(), orc.read_counts())
