@@ -67,10 +67,13 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.index)],
+                                          "-lms", "10", "-i", str(self.index)],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._pump, daemon=True)
             self.th.start()
+            t_end = time.time() + 5.0             # nvidia-smi needs a moment before its first line
+            while len(self.lines) < 2 and time.time() < t_end:
+                time.sleep(0.01)
         except OSError:
             self.proc = None
 
@@ -81,10 +84,14 @@ class ClockSampler:
     def stop(self, t0, t1):
         if not self.proc:
             return None
-        time.sleep(0.15)
+        time.sleep(0.05)
         self.proc.terminate()
-        rows = [l.split(", ") for ts, l in self.lines if t0 - 0.05 <= ts <= t1 + 0.15] or \
-               [l.split(", ") for ts, l in self.lines[-3:]]
+        # samples inside the timed region (10 ms period; a line is stamped when it is read, i.e. slightly late);
+        # a region shorter than the period may hold none: then the samples nearest to it
+        rows = [l.split(", ") for ts, l in self.lines if t0 <= ts <= t1 + 0.03]
+        if not rows:
+            near = sorted(self.lines, key=lambda e: min(abs(e[0] - t0), abs(e[0] - t1)))[:3]
+            rows = [l.split(", ") for ts, l in near]
         sm, reasons, smax = [], set(), None
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in rows:
