@@ -424,6 +424,8 @@ __device__ __forceinline__ void delta_flush(const int32_t* s_delta, uint32_t* __
 // per-thread search.
 constexpr int kPairThreads = 256;
 constexpr unsigned long long kNoKey = ~0ull;
+constexpr int32_t kFarAway = (int32_t)0x80000000;   // x of a slot that holds no agent: practically never inside a window
+                                                   // (and a hit is only queued for slots below the population count)
 
 // Reaction lookup, exact radius and symmetric pair draw for the geometric hit (i, j); on success
 // both ends are merged.
@@ -452,7 +454,7 @@ struct PairWarpSmem {                   // private to one warp
   uint32_t nhit, ntask;
 };
 struct PairSmem {
-  int4 pos[kPairThreads];               // x, y, z, species | forward-row mask << 16
+  int4 pos[kPairThreads + 4];           // x, y, z, species | forward-row mask << 16; 4 far-away sentinels behind
   uint32_t row[kPairThreads], xr[kPairThreads];   // own row's first cell; first x cell | (x cells - 1) << 30
   PairWarpSmem w[kPairThreads / 32];
 };
@@ -464,30 +466,51 @@ __device__ __forceinline__ void push_hit(PairWarpSmem& W, uint32_t owner, uint32
 
 // Tile slots [ka, kb) (shared memory) against the agent `owner` at (x, y, z).
 __device__ __forceinline__ void scan_tile(const Params& p, const PairSmem& S, PairWarpSmem& W, uint32_t ka, uint32_t kb,
-                                          uint32_t base, uint32_t owner, int32_t x, int32_t y, int32_t z) {
+                                          uint32_t base, uint32_t n, uint32_t owner, int32_t x, int32_t y, int32_t z) {
   const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
   const int32_t ox = R - x, oy = R - y, oz = R - z;
-#pragma unroll 4
-  for (uint32_t k = ka; k < kb; ++k) {
-    const int4 q = S.pos[k];
-    const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
-    if (max(max(ux, uy), uz) <= R2) push_hit(W, owner, base + k);   // |d| <= R on every axis: D looks closer
+  // Groups of four candidates, branch-free (one predicate bit each), one branch per group.  A group may run up
+  // to three slots past kb: those belong to cells further on (or to the far-away sentinels behind the tile), fail
+  // the window test unless they are a genuine forward pair of this agent, and a pair queued twice is merged
+  // twice by atomicMin, which changes nothing.
+  for (uint32_t k = ka; k < kb; k += 4u) {
+    uint32_t hits = 0;
+#pragma unroll
+    for (uint32_t u = 0; u < 4u; ++u) {
+      const int4 q = S.pos[k + u];
+      const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
+      hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;       // |d| <= R on every axis: D looks closer
+    }
+    for (; hits; hits &= hits - 1u) {                       // rare
+      const uint32_t j = base + k + (uint32_t)__ffs(hits) - 1u;
+      if (j < n) push_hit(W, owner, j);                      // never a slot past the population
+    }
   }
 }
 
 // Global slots [j0, j1) against the agent `owner` of the tile at (x, y, z).
-__device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, uint32_t j0, uint32_t j1, uint32_t owner,
-                                            int32_t x, int32_t y, int32_t z) {
+__device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, uint32_t j0, uint32_t j1, uint32_t n,
+                                            uint32_t owner, int32_t x, int32_t y, int32_t z) {
   const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
   const int32_t ox = R - x, oy = R - y, oz = R - z;
   const int4* __restrict__ Rr = p.oth.r;
-#pragma unroll 2
-  for (uint32_t j = j0; j < j1; ++j) {
-    const int4 q = __ldg(Rr + j);
-    const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
-    if (max(max(ux, uy), uz) <= R2) push_hit(W, owner, j);
+  // as in scan_tile: groups of four records in flight, branch-free; slots past j1 are later slots of the sorted
+  // array (a genuine forward pair if they pass) or past the population (never queued: j < n), and the record
+  // array has slack for the three records a group may read past its end
+  for (uint32_t j = j0; j < j1; j += 4u) {
+    uint32_t hits = 0;
+#pragma unroll
+    for (uint32_t u = 0; u < 4u; ++u) {
+      const int4 q = __ldg(Rr + j + u);
+      const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
+      hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;
+    }
+    for (; hits; hits &= hits - 1u) {
+      const uint32_t jj = j + (uint32_t)__ffs(hits) - 1u;
+      if (jj < n) push_hit(W, owner, jj);
+    }
   }
 }
 
@@ -540,6 +563,7 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
   uint32_t s = kDead;
   int32_t x = 0, y = 0, z = 0;
   if (i < n) { s = p.oth.sp[i]; const int4 q = p.oth.r[i]; x = q.x; y = q.y; z = q.z; }
+  else x = kFarAway;                                  // a slot past the population
   const bool active = s != kDead && ((p.binds_mask >> s) & 1ull);
   uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0, j1 = 0;
   if (active) {
@@ -557,12 +581,13 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
   }
   S.pos[tid] = make_int4(x, y, z, (int32_t)(s | (need << 16)));    // species | forward-row mask << 16
   S.row[tid] = rowc; S.xr[tid] = xlo | (nxr << 30);
+  if (tid < 4u) S.pos[kPairThreads + tid] = make_int4(kFarAway, 0, 0, (int32_t)kDead);
   __syncthreads();          // the only block-wide barrier: the tile is read-only from here on
 
   // ---- A: own row, slots (i, j1)
   if (active) {
-    scan_tile(p, S, W, tid + 1u, min(j1, base + kPairThreads) - base, base, tid, x, y, z);
-    if (j1 > base + kPairThreads) scan_global(p, W, base + kPairThreads, j1, tid, x, y, z);
+    scan_tile(p, S, W, tid + 1u, min(j1, base + kPairThreads) - base, base, n, tid, x, y, z);
+    if (j1 > base + kPairThreads) scan_global(p, W, base + kPairThreads, j1, n, tid, x, y, z);
   }
 
   // ---- B: the warp's task list: the ~20 % of lanes that face a +y / +z cell append their forward rows
@@ -584,7 +609,7 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
       const uint32_t r2 = S.row[owner] + (uint32_t)p.fwd_row[(e >> 8) - 5u];   // host-precomputed row offsets of codes 5..8
       const int4 q = S.pos[owner];
       const uint32_t j0 = p.cell[r2 + oxlo], len = p.cell[r2 + oxlo + onx + 1] - j0;
-      scan_global(p, W, j0 + ((len * part) >> lg), j0 + ((len * (part + 1u)) >> lg), owner, q.x, q.y, q.z);
+      scan_global(p, W, j0 + ((len * part) >> lg), j0 + ((len * (part + 1u)) >> lg), n, owner, q.x, q.y, q.z);
     }
   }
   __syncwarp();
