@@ -2,7 +2,7 @@
 // Product code (CUDA path).  Shares nothing with oracle/.
 //
 // One step = K1 move+hist -> K2 cell scan (2 launches) -> K3 move+scatter -> K4 pair search/proposal ->
-// K4b resolve -> K5 unimolecular -> K6 birth scan (2 launches) + birth placement -> K7 epilogue.
+// K4b resolve -> K5 unimolecular -> K6 births (ranking + placement, 1 launch) -> K7 epilogue: 10 launches.
 // Every decision is keyed by agent id (never by slot), so the nondeterministic slot order the
 // histogram atomics produce inside a cell cannot change any result.
 #pragma once
