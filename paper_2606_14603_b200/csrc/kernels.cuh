@@ -593,9 +593,11 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
   // ---- B: the warp's task list: the ~20 % of lanes that face a +y / +z cell append their forward rows
   // (order is irrelevant: every hit is merged by atomicMin)
   if (need >> 5) {
-    uint32_t m = need >> 5;
-    uint32_t pos = atomicAdd(&W.ntask, (uint32_t)__popc(m));
-    for (; m; m &= m - 1u) W.task[pos++] = (uint16_t)(tid | ((uint32_t)(__ffs(m) + 4) << 8));
+    const uint32_t m = need >> 5;
+    const uint32_t pos = atomicAdd(&W.ntask, (uint32_t)__popc(m));
+#pragma unroll
+    for (uint32_t c = 0; c < 4u; ++c)      // four predicated stores instead of a data-dependent loop
+      if (m >> c & 1u) W.task[pos + __popc(m & ((1u << c) - 1u))] = (uint16_t)(tid | ((c + 5u) << 8));
   }
   __syncwarp();
   const uint32_t nt = W.ntask;
