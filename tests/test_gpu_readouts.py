@@ -144,3 +144,30 @@ def test_compiled_physical_model_parity(gpu):
     for k in ("id", "species", "x", "y", "z"):
         assert np.array_equal(a[k], b[k]), k
     assert np.array_equal(sim.read_counts(), orc.read_counts())
+
+
+def test_derived_concentration_curves_and_perk_fraction(gpu):
+    """SURVEY 8(a) a11 / [NS]: the only floating-point outputs are derived on the host in double from the integer
+    counts — concentration curves c(t) = n(t) / (N_A V) and [CFG 2]'s steady-state pERK fraction (reading S19) — and
+    are held to a relative tolerance of 1e-6 against the same derivation from the oracle's counts."""
+    from oracle.binding import Oracle
+    from workloads import model as wm
+
+    m = configs.w2(scale=0.002, n_steps=120)
+    sim, orc = gpu.Sim(m), Oracle(m)
+    for s in (sim, orc):
+        s.seed_population(); s.step(120)
+    cg, co = sim.read_counts(), orc.read_counts()
+    curves_g = wm.concentration_molar(cg, m.volume_um3)
+    curves_o = wm.concentration_molar(co, m.volume_um3)
+    assert curves_g.dtype == np.float64 and curves_g.shape == cg.shape
+    nz = curves_o != 0
+    assert np.all(np.abs(curves_g[nz] - curves_o[nz]) <= 1e-6 * np.abs(curves_o[nz])) and np.all(curves_g[~nz] == 0)
+    names = [s.name for s in m.species]
+    perk, erk_like = names.index("pERK"), [names.index(n) for n in ("ERK", "pERK", "pMEK:ERK", "P:pERK")]
+    frac_g = cg[-50:, :, perk].mean(axis=0) / cg[0][:, erk_like].sum(axis=1)
+    frac_o = co[-50:, :, perk].mean(axis=0) / co[0][:, erk_like].sum(axis=1)
+    assert np.allclose(frac_g, frac_o, rtol=1e-6, atol=0.0)
+    # closed form: one molecule in the replica volume
+    one = wm.concentration_molar(np.array([1]), m.volume_um3)[0]
+    assert abs(one * wm.N_AVOGADRO * m.volume_um3 * 1e-15 - 1.0) < 1e-12
