@@ -414,7 +414,7 @@ def run_gpu(args):
         "dtype": "int32", "data": "synthetic",
         "config": {"workload": workload_name(args, m), "n_live_mean": n_live_mean,
                    "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)",
-                   "l2": "inputs larger than L2 (SoA ping-pong %.0f MB vs 126 MB L2), no flush" %
+                   "l2": "inputs larger than L2 (agent-store ping-pong %.0f MB vs 126 MB L2), no flush" %
                          (2 * BYTES_PER_AGENT * n_live_mean / 1e6),
                    "bytes_per_agent_step_ledger": round(step_bytes / n_live_mean, 1),
                    "bytes_per_agent_step_moved": round(moved_bytes / n_live_mean, 1)},

@@ -272,7 +272,7 @@ bool capture_steps(sim* s, uint32_t steps, cudaGraphExec_t* out) {
   return ok;
 }
 
-// The 12 launches of a step are replayed as CUDA graphs (one step, or 8 steps, per starting parity of
+// The 10 launches of a step are replayed as CUDA graphs (one step, or 8 steps, per starting parity of
 // the cur/oth ping-pong): the path is launch-bound below ~1 M agents.
 void build_graphs(sim* s) {
   s->graphs_tried = true;
