@@ -398,238 +398,252 @@ __device__ __forceinline__ void delta_flush(const int32_t* s_delta, uint32_t* __
 // ----------------------------------------------------------------------------- K4 pair search + proposal
 // Phase 2a: each agent whose species can bind proposes its eligible partner with the smallest
 // (dist^2, id) among those that pass the symmetric pair draw (a6).  The predicate and the draw are
-// symmetric in the pair, so every unordered pair is examined ONCE, by its lower sorted slot i < j,
+// symmetric in the pair, so every unordered pair is examined ONCE, from its lower sorted slot i < j,
 // and a qualifying pair is merged into both ends: best[i] <- min(., (d2, id_j)), best[j] <- min(.,
-// (d2, id_i)) with 64-bit global atomicMin.  Only cells the R-ball overlaps are visited (exact: a
+// (d2, id_i)) with 64-bit global atomic min.  Only cells the R-ball overlaps are visited (exact: a
 // cell it does not overlap cannot hold an in-range partner), and of those only the "forward" ones:
 // the rest of the agent's own cell, the +x cell, and the overlapped cells of the rows (y+1, z) and
 // (y-1..y+1, z+1).  With x-fastest cell keys the cells of one (y,z) row are one contiguous slot range.
 //
-// Work layout.  A block owns a tile of 256 consecutive sorted slots and stages their positions in
-// shared memory as int4 (x, y, z, species); after that single barrier its warps work on their own:
-//  A  own row: slots (i, j1).  Inside the tile: one 128-bit shared load, three adds, two max and one
-//     compare per candidate, no branch unless all three axes are within R; the few slots past the
-//     tile end are read from global memory.
-//  B  the forward (y,z) rows, which only agents near a +y / +z (or, for the z+1 rows, -y) cell face
-//     need, are pushed as 16-bit tasks (owner, row code) into the warp's shared list and
-//  C  scanned by the whole warp, 1, 2 or 4 lanes per task, so the few lanes that need them do not
-//     stall the others.
-//  D  window hits (|d| <= R on every axis: a fraction of a percent of the candidates) were only queued;
-//     now one lane per hit does the exact distance, the reaction lookup and the pair draw and, if the pair qualifies,
-//     the two atomicMin.  best[] is touched only there (rare), so it costs no bandwidth; hasprop
-//     gets one bit per touched agent and bslot[] the slot of the partner that lowered the key.
-//     Two lanes lowering the same key may store their slots in either order, so K4b checks
-//     id[bslot[i]] against the key and searches the neighbourhood again in that (vanishingly rare) case.
-// A warp with more hits than its queue holds (dense test inputs) redoes its agents by a plain
-// per-thread search.
+// Work layout (round 2; profiles/r2_pairs.md has the per-phase instruction split that led here: set-up,
+// divergent row visits and one-lane hit qualification were 70 % of the instructions, and a first cut with
+// per-tile block queues was bound by the barrier before the rare work).  The kernel is persistent: a
+// block walks tiles of 256 consecutive sorted slots; the records of the NEXT tile (plus kPairHalo slots
+// behind it) and its species arrive in shared memory by two bulk copies (cp.async.bulk + mbarrier, the
+// TMA engine) while the current tile is worked on, so no warp ever waits on the streaming loads.
+// Per tile every warp does dense work only:
+//  A  own row.  Every agent tests the kPairWin slots behind its own straight from shared memory: no
+//     range look-up, no loop, every lane busy.  A slot that passes the window test (|d| <= R on every
+//     axis) is a genuine close pair whatever cell it lies in, so nothing has to bound the window; the
+//     own-row range (rest of the own cell, plus the +x cell if the R-ball reaches it) is longer than
+//     the window only if the slot right behind the window still lies in that x interval: then the
+//     remainder becomes a task.
+//  B  agents that face a +y / +z cell (about a fifth) append one 8-byte task per forward row (owner
+//     slot, first cell of the range, cells in it) to the block's task queue; window hits go to the block's hit
+//     queue as (i, j, id_j, d2).
+// The rare work is DEFERRED until a block's worth of it has piled up (every few tiles), so that it too runs
+// with every lane busy and its look-up latency is paid once per batch instead of once per tile:
+//  C  task drain: one thread per task: two cell-range look-ups, then records in groups of four.
+//  D  hit drain: one thread per hit: reaction look-up, exact radius, symmetric pair draw and, if the pair
+//     qualifies, the two atomic mins.  best[] is touched only there (rare), so it costs no bandwidth;
+//     hasprop gets one bit per touched agent and prop[] the slot of a partner that qualified.  prop[] is a
+//     plain store (no round trip for the old key): with several qualifying partners it may name another than the
+//     minimum, so K4b checks id[prop[i]] against the key and searches the neighbourhood again in that
+//     (rare) case.  A pair reached twice (window and row) is merged twice, which changes nothing.
+// The task queue holds a drain mark's worth plus a whole tile (at most five tasks per agent), so it cannot
+// overflow; a hit that finds its queue full (dense test inputs) is qualified on the spot by the thread that found it.
 constexpr int kPairThreads = 256;
+constexpr int kPairWin = 8;             // slots behind its own that every agent tests in phase A
+constexpr int kPairHalo = 16;           // slots staged behind the tile: kPairWin + the over-run probe, rounded up
+constexpr int kPairTaskDrain = 256;                        // a block's worth of tasks: drain before the next tile
+constexpr int kPairTaskCap = kPairTaskDrain + 5 * kPairThreads;   // ... so a tile (<= 5 tasks per agent) always fits
+constexpr int kPairHitCap = 128, kPairHitDrain = 64;
+constexpr uint32_t kPairTileBytes = (kPairThreads + kPairHalo) * 16u + kPairThreads * 2u;
 constexpr unsigned long long kNoKey = ~0ull;
-constexpr int32_t kFarAway = (int32_t)0x80000000;   // x of a slot that holds no agent: practically never inside a window
-                                                   // (and a hit is only queued for slots below the population count)
 
-// Reaction lookup, exact radius and symmetric pair draw for the geometric hit (i, j); on success
-// both ends are merged.
-__device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t j, uint32_t d2, uint32_t si, uint32_t t) {
+// ---- mbarrier + bulk copy (PTX, sm_90+; SASS on sm_100a: SYNCS / UBLKCP)
+__device__ __forceinline__ uint32_t smem_addr(const void* ptr) { return (uint32_t)__cvta_generic_to_shared(ptr); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
+  return ok != 0u;
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+
+struct PairSmem {
+  int4 rec[2][kPairThreads + kPairHalo];   // x, y, z, id of the tile's slots and the kPairHalo behind them
+  uint16_t sp[2][kPairThreads];            // species
+  uint2 task[kPairTaskCap];                // owner slot, first cell | (cells - 1) << 30   (3: own-row remainder)
+  uint4 hit[kPairHitCap];                  // i, j, id_j, d2
+  unsigned long long bar[2];
+  uint32_t ntask, nhit;
+};
+
+// Reaction look-up, exact radius and symmetric pair draw for the geometric hit (i, j); on success both ends are merged.
+__device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t j, uint32_t idj, uint32_t d2) {
   const DevTables* __restrict__ T = p.tab;
-  const uint32_t e = T->rxmap[si * kMaxSpecies + p.oth.sp[j]];
+  const uint32_t si = p.oth.sp[i], sj = p.oth.sp[j], id = (uint32_t)p.oth.r[i].w;
+  const uint32_t e = T->rxmap[si * kMaxSpecies + sj];
   if (e == 0xFFu) return;
   const DevRx& rx = T->rx[e];
   if (d2 > rx.r2) return;
-  const uint32_t id = (uint32_t)p.oth.r[i].w, idj = (uint32_t)p.oth.r[j].w;
-  const uint4 r = philox_sim(p, min(id, idj), max(id, idj), t, kTagPair);
+  const uint4 r = philox_sim(p, min(id, idj), max(id, idj), p.scal->t, kTagPair);
   if (!fire(r.x, rx.thr)) return;
-  const unsigned long long hi = (unsigned long long)d2 << 32, ki = hi | idj, kj = hi | id;
-  if (atomicMin(&p.best[i], ki) > ki) p.prop[i] = j;
-  if (atomicMin(&p.best[j], kj) > kj) p.prop[j] = i;
+  const unsigned long long hi = (unsigned long long)d2 << 32;
+  atomicMin(&p.best[i], hi | idj);
+  atomicMin(&p.best[j], hi | id);
+  p.prop[i] = j; p.prop[j] = i;
   atomicOr(&p.hasprop[i >> 5], 1u << (i & 31u));
   atomicOr(&p.hasprop[j >> 5], 1u << (j & 31u));
 }
 
-constexpr int kWarpTaskCap = 128;       // 4 forward rows x 32 agents: always fits
-constexpr int kWarpHitCap = 64;
-struct PairWarpSmem {                   // private to one warp
-  uint32_t hit_j[kWarpHitCap];          // candidate slot that passed the window test
-  uint8_t hit_o[kWarpHitCap];           // owner thread
-  uint16_t task[kWarpTaskCap];          // owner thread | row code (5..8) << 8
-  uint32_t nhit, ntask;
-};
-struct PairSmem {
-  int4 pos[kPairThreads + 4];           // x, y, z, species | forward-row mask << 16; 4 far-away sentinels behind
-  uint32_t row[kPairThreads], xr[kPairThreads];   // own row's first cell; first x cell | (x cells - 1) << 30
-  PairWarpSmem w[kPairThreads / 32];
-};
-
-__device__ __forceinline__ void push_hit(PairWarpSmem& W, uint32_t owner, uint32_t j) {
-  const uint32_t h = atomicAdd(&W.nhit, 1u);
-  if (h < (uint32_t)kWarpHitCap) { W.hit_j[h] = j; W.hit_o[h] = (uint8_t)owner; }
+__device__ __noinline__ void pair_merge_now(const Params* p, uint32_t i, uint32_t j, uint32_t idj, uint32_t d2) {
+  pair_merge(*p, i, j, idj, d2);
+}
+// Returns true when the hit queue has reached its drain mark.  A hit that finds the queue full (dense test
+// inputs) is qualified on the spot.
+__device__ __forceinline__ bool push_hit(const Params& p, PairSmem& S, uint32_t i, uint32_t j, uint32_t idj, uint32_t d2) {
+  const uint32_t h = atomicAdd(&S.nhit, 1u);
+  if (h < (uint32_t)kPairHitCap) S.hit[h] = make_uint4(i, j, idj, d2);
+  else pair_merge_now(&p, i, j, idj, d2);
+  return h + 1u >= (uint32_t)kPairHitDrain;
 }
 
-// Tile slots [ka, kb) (shared memory) against the agent `owner` at (x, y, z).
-__device__ __forceinline__ void scan_tile(const Params& p, const PairSmem& S, PairWarpSmem& W, uint32_t ka, uint32_t kb,
-                                          uint32_t base, uint32_t n, uint32_t owner, int32_t x, int32_t y, int32_t z) {
-  const int32_t R = p.max_r;
-  const uint32_t R2 = 2u * (uint32_t)R;
-  const int32_t ox = R - x, oy = R - y, oz = R - z;
-  // Groups of four candidates, branch-free (one predicate bit each), one branch per group.  A group may run up
-  // to three slots past kb: those belong to cells further on (or to the far-away sentinels behind the tile), fail
-  // the window test unless they are a genuine forward pair of this agent, and a pair queued twice is merged
-  // twice by atomicMin, which changes nothing.
-  for (uint32_t k = ka; k < kb; k += 4u) {
-    uint32_t hits = 0;
-#pragma unroll
-    for (uint32_t u = 0; u < 4u; ++u) {
-      const int4 q = S.pos[k + u];
-      const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
-      hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;       // |d| <= R on every axis: D looks closer
-    }
-    for (; hits; hits &= hits - 1u) {                       // rare
-      const uint32_t j = base + k + (uint32_t)__ffs(hits) - 1u;
-      if (j < n) push_hit(W, owner, j);                      // never a slot past the population
-    }
-  }
-}
-
-// Global slots [j0, j1) against the agent `owner` of the tile at (x, y, z).
-__device__ __forceinline__ void scan_global(const Params& p, PairWarpSmem& W, uint32_t j0, uint32_t j1, uint32_t n,
-                                            uint32_t owner, int32_t x, int32_t y, int32_t z) {
+// Global slots [j0, j1) against agent i at (x, y, z).
+__device__ __forceinline__ bool scan_rows(const Params& p, PairSmem& S, uint32_t j0, uint32_t j1, uint32_t n,
+                                          uint32_t i, int32_t x, int32_t y, int32_t z) {
+  bool full = false;
   const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
   const int32_t ox = R - x, oy = R - y, oz = R - z;
   const int4* __restrict__ Rr = p.oth.r;
-  // as in scan_tile: groups of four records in flight, branch-free; slots past j1 are later slots of the sorted
-  // array (a genuine forward pair if they pass) or past the population (never queued: j < n), and the record
-  // array has slack for the three records a group may read past its end
+  // groups of four records in flight, branch-free (one predicate bit each), one branch per group.  A group
+  // may run up to three slots past j1: those are later slots of the sorted array (a genuine forward pair if
+  // they pass) or past the population (never queued: j < n); the record array has slack for them
   for (uint32_t j = j0; j < j1; j += 4u) {
     uint32_t hits = 0;
 #pragma unroll
     for (uint32_t u = 0; u < 4u; ++u) {
       const int4 q = __ldg(Rr + j + u);
       const uint32_t ux = (uint32_t)(q.x + ox), uy = (uint32_t)(q.y + oy), uz = (uint32_t)(q.z + oz);
-      hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;
+      hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;    // |d| <= R on every axis
     }
-    for (; hits; hits &= hits - 1u) {
+    for (; hits; hits &= hits - 1u) {                       // rare
       const uint32_t jj = j + (uint32_t)__ffs(hits) - 1u;
-      if (jj < n) push_hit(W, owner, jj);
-    }
-  }
-}
-
-// Linear index of cell (0, y + dy, z + dz) for row code c = (dz+1)*3 + (dy+1).
-__device__ __forceinline__ uint32_t row_of(const Params& p, uint32_t rowc, uint32_t c) {
-  const int32_t dz = c >= 6u ? 1 : (c >= 3u ? 0 : -1);
-  const int32_t dy = (int32_t)c - 3 * dz - 4;
-  return rowc + (uint32_t)((dz * p.ny + dy) * p.nx);
-}
-
-// Plain per-thread forward search with immediate merge: used by warps whose hit queue overflowed.
-// Everything it needs is read back from the tile in shared memory, so the fast path keeps no
-// registers alive for it.
-__device__ __noinline__ void slow_agent(const Params* pp, const PairSmem* Sp, uint32_t tid, uint32_t i, uint32_t t) {
-  const Params& p = *pp;
-  const int4 q = Sp->pos[tid];
-  const int32_t x = q.x, y = q.y, z = q.z;
-  const uint32_t si = (uint32_t)q.w & 0xFFFFu, rowc = Sp->row[tid], xr = Sp->xr[tid];
-  const uint32_t xlo = xr & 0x3FFFFFFFu, nxr = xr >> 30;
-  uint32_t need = ((uint32_t)q.w >> 16) | (1u << 4);
-  const long long R = p.max_r;
-  while (need) {
-    const uint32_t c = __ffs(need) - 1u;
-    need &= need - 1u;
-    const uint32_t r2 = row_of(p, rowc, c);
-    const uint32_t j0 = c == 4u ? i + 1u : p.cell[r2 + xlo], j1 = p.cell[r2 + xlo + nxr + 1];
-    for (uint32_t j = j0; j < j1; ++j) {
-      const int4 qj = p.oth.r[j];
-      const long long dx = (long long)qj.x - x, dy = (long long)qj.y - y, dz = (long long)qj.z - z;
-      if (dx > R || dx < -R || dy > R || dy < -R || dz > R || dz < -R) continue;
-      const unsigned long long d2 = (unsigned long long)(dx * dx + dy * dy + dz * dz);
-      if (d2 <= p.max_r2) pair_merge(p, i, j, (uint32_t)d2, si, t);
-    }
-  }
-}
-
-#ifndef MOLSIM_PAIR_MINBLK
-#define MOLSIM_PAIR_MINBLK 8      // measured on B200: 4/5/6/8 blocks per SM -> 0.46 / 0.41 / 0.35 / 0.31 ms at 16 M agents
-#endif
-__global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(const __grid_constant__ Params p) {
-  __shared__ PairSmem S;
-  const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
-  const uint32_t base = blockIdx.x * kPairThreads;
-  if (base >= n) return;
-  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, tid = threadIdx.x;
-  PairWarpSmem& W = S.w[warp];
-  const int32_t R = p.max_r, cs = p.cell_size;
-  if (lane == 0) { W.nhit = 0; W.ntask = 0; }
-  const uint32_t i = base + tid;
-  uint32_t s = kDead;
-  int32_t x = 0, y = 0, z = 0;
-  if (i < n) { s = p.oth.sp[i]; const int4 q = p.oth.r[i]; x = q.x; y = q.y; z = q.z; }
-  else x = kFarAway;                                  // a slot past the population
-  const bool active = s != kDead && ((p.binds_mask >> s) & 1ull);
-  uint32_t rowc = 0, xlo = 0, nxr = 0, need = 0, j1 = 0;
-  if (active) {
-    // R <= cell_size (validated), so the R-ball reaches at most one cell further on each side
-    const int32_t cx = cell_coord(x, p), cy = cell_coord(y, p), cz = cell_coord(z, p);
-    const int32_t lx = x - cx * cs, ly = y - cy * cs, lz = z - cz * cs;
-    const uint32_t xm = lx < R && cx > 0, xp = lx >= cs - R && cx < p.nx - 1;
-    const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
-    const uint32_t zp = lz >= cs - R && cz < p.nz - 1;
-    xlo = (uint32_t)cx - xm; nxr = xm + xp;
-    rowc = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx;
-    // forward rows, bit (dz+1)*3 + (dy+1): (y+1, z) = 5; (y-1, z+1), (y, z+1), (y+1, z+1) = 6, 7, 8
-    need = (yp << 5) | (zp ? ((ym | 2u | (yp << 2)) << 6) : 0u);
-    j1 = p.cell[rowc + (uint32_t)cx + xp + 1u];            // end of the own-row forward range, > i
-  }
-  S.pos[tid] = make_int4(x, y, z, (int32_t)(s | (need << 16)));    // species | forward-row mask << 16
-  S.row[tid] = rowc; S.xr[tid] = xlo | (nxr << 30);
-  if (tid < 4u) S.pos[kPairThreads + tid] = make_int4(kFarAway, 0, 0, (int32_t)kDead);
-  __syncthreads();          // the only block-wide barrier: the tile is read-only from here on
-
-  // ---- A: own row, slots (i, j1)
-  if (active) {
-    scan_tile(p, S, W, tid + 1u, min(j1, base + kPairThreads) - base, base, n, tid, x, y, z);
-    if (j1 > base + kPairThreads) scan_global(p, W, base + kPairThreads, j1, n, tid, x, y, z);
-  }
-
-  // ---- B: the warp's task list: the ~20 % of lanes that face a +y / +z cell append their forward rows
-  // (order is irrelevant: every hit is merged by atomicMin)
-  if (need >> 5) {
-    const uint32_t m = need >> 5;
-    const uint32_t pos = atomicAdd(&W.ntask, (uint32_t)__popc(m));
-#pragma unroll
-    for (uint32_t c = 0; c < 4u; ++c)      // four predicated stores instead of a data-dependent loop
-      if (m >> c & 1u) W.task[pos + __popc(m & ((1u << c) - 1u))] = (uint16_t)(tid | ((c + 5u) << 8));
-  }
-  __syncwarp();
-  const uint32_t nt = W.ntask;
-
-  // ---- C: the forward rows: 4, 2 or 1 lanes per task
-  {
-    const uint32_t lg = nt <= 8u ? 2u : (nt <= 16u ? 1u : 0u), items = nt << lg;
-    for (uint32_t k = lane; k < items; k += 32u) {
-      const uint32_t e = W.task[k >> lg], owner = e & 0xFFu, part = k & ((1u << lg) - 1u);
-      const uint32_t xr = S.xr[owner], oxlo = xr & 0x3FFFFFFFu, onx = xr >> 30;
-      const uint32_t r2 = S.row[owner] + (uint32_t)p.fwd_row[(e >> 8) - 5u];   // host-precomputed row offsets of codes 5..8
-      const int4 q = S.pos[owner];
-      const uint32_t j0 = p.cell[r2 + oxlo], len = p.cell[r2 + oxlo + onx + 1] - j0;
-      scan_global(p, W, j0 + ((len * part) >> lg), j0 + ((len * (part + 1u)) >> lg), n, owner, q.x, q.y, q.z);
-    }
-  }
-  __syncwarp();
-
-  // ---- D: qualify the queued hits, one lane per hit: exact distance, then reaction look-up and draw
-  const uint32_t nh = W.nhit;
-  if (nh <= (uint32_t)kWarpHitCap) {
-    for (uint32_t h = lane; h < nh; h += 32u) {
-      const uint32_t owner = W.hit_o[h], j = W.hit_j[h];
-      const int4 q = S.pos[owner];
-      const int4 qj = p.oth.r[j];
-      const int32_t dx = qj.x - q.x, dy = qj.y - q.y, dz = qj.z - q.z;   // each within +-R
+      const int4 q = __ldg(Rr + jj);
+      const int32_t dx = q.x - x, dy = q.y - y, dz = q.z - z;     // each within +-R
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (d2 <= p.max_r2) pair_merge(p, base + owner, j, d2, (uint32_t)q.w & 0xFFFFu, t);
+      if (jj < n && d2 <= p.max_r2) full |= push_hit(p, S, i, jj, (uint32_t)q.w, d2);
     }
-  } else if (active) {
-    slow_agent(&p, &S, tid, i, t);
   }
+  return full;
+}
+
+__device__ __forceinline__ void pair_issue_tile(const Params& p, PairSmem& S, uint32_t buf, uint32_t tile) {
+  // generic-proxy reads of this buffer (two tiles ago) are ordered before the async-proxy refill
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  mbar_expect_tx(&S.bar[buf], kPairTileBytes);
+  bulk_g2s(S.rec[buf], p.oth.r + (size_t)tile * kPairThreads, (kPairThreads + kPairHalo) * 16u, &S.bar[buf]);
+  bulk_g2s(S.sp[buf], p.oth.sp + (size_t)tile * kPairThreads, kPairThreads * 2u, &S.bar[buf]);
+}
+
+// C / D: drain the block's queues (called by every thread of the block).  Nobody appends tasks in here, and hits
+// are appended only before the first barrier, so the counters read below are the same for every thread.
+// Kept out of line: its registers (Philox, 64-bit keys) must not be charged to the dense per-tile loop.
+__device__ __noinline__ void pair_drain(const Params* pp, PairSmem* Sp, uint32_t n, bool all) {
+  const Params& p = *pp;
+  PairSmem& S = *Sp;
+  const uint32_t nt = S.ntask;
+  const bool dt = all || nt >= (uint32_t)kPairTaskDrain;
+  if (dt) {
+    for (uint32_t k = threadIdx.x; k < nt; k += kPairThreads) {     // one thread per task
+      const uint2 tk = S.task[k];
+      const int4 o = __ldg(p.oth.r + tk.x);
+      const uint32_t c0 = tk.y & 0x3FFFFFFFu, nc = tk.y >> 30;    // first cell | (cells - 1) << 30, or own-row remainder
+      uint32_t j0, j1;
+      if (nc == 3u) { j0 = tk.x + 1u + (uint32_t)kPairWin; j1 = p.cell[c0 + 1u]; }    // c0 = last cell of the own-row range
+      else { j0 = p.cell[c0]; j1 = p.cell[c0 + nc + 1u]; }
+      scan_rows(p, S, j0, j1, n, tk.x, o.x, o.y, o.z);
+    }
+  }
+  __syncthreads();
+  const uint32_t nh = min(S.nhit, (uint32_t)kPairHitCap);
+  const bool dh = all || nh >= (uint32_t)kPairHitDrain;
+  if (dh) {
+    for (uint32_t h = threadIdx.x; h < nh; h += kPairThreads) {     // one thread per hit
+      const uint4 e = S.hit[h];
+      pair_merge(p, e.x, e.y, e.z, e.w);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) { if (dt) S.ntask = 0; if (dh) S.nhit = 0; }
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(kPairThreads, 4) k_pairs(const __grid_constant__ Params p) {
+  __shared__ __align__(128) PairSmem S;
+  const uint32_t n = p.cell[p.n_cells];
+  const uint32_t ntiles = (n + kPairThreads - 1u) / kPairThreads;
+  if (blockIdx.x >= ntiles) return;
+  const uint32_t tid = threadIdx.x;
+  if (tid == 0) {
+    S.ntask = 0; S.nhit = 0;
+    mbar_init(&S.bar[0], 1u); mbar_init(&S.bar[1], 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    pair_issue_tile(p, S, 0u, blockIdx.x);
+  }
+  __syncthreads();
+  const int32_t R = p.max_r, cs = p.cell_size;
+  const uint32_t R2 = 2u * (uint32_t)R;
+  uint32_t it = 0;
+  bool drain = false;        // block-uniform: a queue reached its drain mark during the previous tile
+  for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+    const uint32_t buf = it & 1u;
+    // ---- C / D: drain the queues once a block's worth has piled up
+    if (drain) pair_drain(&p, &S, n, false);
+    // next tile -> the other buffer (its readers finished before the barrier that ended the previous tile)
+    if (tid == 0 && tile + gridDim.x < ntiles) pair_issue_tile(p, S, buf ^ 1u, tile + gridDim.x);
+    while (!mbar_try_wait(&S.bar[buf], (it >> 1) & 1u)) {}
+    const uint32_t i = tile * kPairThreads + tid;
+    const int4 q = S.rec[buf][tid];
+    const uint32_t s = S.sp[buf][tid];
+    bool want = false;       // this thread saw a queue reach its drain mark
+    if (i < n && s != kDead && ((p.binds_mask >> s) & 1ull)) {
+      // where the agent sits in the cell grid.  R <= cell_size (validated), so its R-ball reaches at most one cell
+      // further on each side
+      const int32_t cx = cell_coord(q.x, p), cy = cell_coord(q.y, p), cz = cell_coord(q.z, p);
+      const int32_t lx = q.x - cx * cs, ly = q.y - cy * cs, lz = q.z - cz * cs;
+      const uint32_t xm = lx < R && cx > 0, xp = lx >= cs - R && cx < p.nx - 1;
+      const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
+      const uint32_t zp = lz >= cs - R && cz < p.nz - 1;
+      // forward rows, bit (dz+1)*3 + (dy+1): (y+1, z) = 5; (y-1, z+1), (y, z+1), (y+1, z+1) = 6, 7, 8; 4 = own-row remainder
+      uint32_t rows = (yp << 5) | (zp ? ((ym | 2u | (yp << 2)) << 6) : 0u);
+      // ---- A: the kPairWin slots behind its own
+      const int32_t ox = R - q.x, oy = R - q.y, oz = R - q.z;
+      uint32_t hits = 0;
+#pragma unroll
+      for (uint32_t u = 0; u < (uint32_t)kPairWin; ++u) {
+        const int4 c = S.rec[buf][tid + 1u + u];
+        const uint32_t ux = (uint32_t)(c.x + ox), uy = (uint32_t)(c.y + oy), uz = (uint32_t)(c.z + oz);
+        hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;
+      }
+      for (; hits; hits &= hits - 1u) {                    // rare
+        const uint32_t u = (uint32_t)__ffs(hits);
+        const int4 c = S.rec[buf][tid + u];
+        const int32_t dx = c.x - q.x, dy = c.y - q.y, dz = c.z - q.z;
+        const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
+        if (i + u < n && d2 <= p.max_r2) want |= push_hit(p, S, i, i + u, (uint32_t)c.w, d2);   // never a slot past the population
+      }
+      // the own-row range goes on behind the window iff the next slot still lies in its x interval (slots of a row
+      // are ordered by x cell; a slot of a LATER row that happens to lie in the interval only costs a look-up)
+      if ((uint32_t)(S.rec[buf][tid + 1u + kPairWin].x - cx * cs) < (1u + xp) * (uint32_t)cs) rows |= 1u << 4;
+      // ---- B: one task per row to visit (order is irrelevant: every hit is merged by atomic min)
+      if (rows) {
+        const uint32_t c0 = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx + (uint32_t)cx;   // own cell
+        const uint32_t fv = (c0 - xm) | ((xm + xp) << 30);         // cells cx - xm .. cx + xp of a forward row
+        uint32_t pos = atomicAdd(&S.ntask, (uint32_t)__popc(rows));   // < kPairTaskDrain before the tile: a tile always fits
+        if (rows & 16u) S.task[pos++] = make_uint2(i, (c0 + xp) | (3u << 30));
+        if (rows & 32u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[0]);
+        if (rows & 64u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[1]);
+        if (rows & 128u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[2]);
+        if (rows & 256u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[3]);
+        want |= pos >= (uint32_t)kPairTaskDrain;
+      }
+    }
+    // rec[buf] may be refilled, the queue counters are final for this tile, and every thread learns whether to drain
+    drain = __syncthreads_or(want);
+  }
+  pair_drain(&p, &S, n, true);
 }
 
 // ----------------------------------------------------------------------------- K4b handshake resolve
@@ -639,7 +653,7 @@ __global__ void __launch_bounds__(kPairThreads, MOLSIM_PAIR_MINBLK) k_pairs(cons
 // kernel: a third agent that proposed to one of them only reads best[] / bslot[].
 
 // Slot of the agent with id `idj` at squared distance d2 from agent i (it exists): the plain
-// neighbourhood sweep, used only when bslot[i] lost a store race (see K4, D).
+// neighbourhood sweep, used only when prop[i] names another qualifying partner than the minimum (see K4, D).
 __device__ __noinline__ uint32_t find_partner(const Params* pp, uint32_t i, uint32_t idj) {
   const Params& p = *pp;
   const int4 qi = p.oth.r[i];

@@ -37,12 +37,13 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   const uint64_t cs = c->cell_size;
   const uint64_t nx = (c->extent[0] + cs - 1) / cs, ny = (c->extent[1] + cs - 1) / cs, nz = (c->extent[2] + cs - 1) / cs;
   const uint64_t nc = nx * ny * nz;
-  if (nc == 0 || nc >= 0x7FFFFFF0ull || nx >= (1ull << 30)) return false;
+  if (nc == 0 || nc >= (1ull << 30) - 8 || nx >= (1ull << 30)) return false;   // K4 packs a cell index into 30 bits
   L.nx = (uint32_t)nx; L.ny = (uint32_t)ny; L.nz = (uint32_t)nz; L.n_cells = (uint32_t)nc;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
   const size_t cap = c->capacity;
-  for (int b = 0; b < 2; ++b) { L.soa[b][0] = take(cap * 16 + 64); L.soa[b][1] = take(cap * 2 + 64); }   // records, species
+  // records, species; the slack covers the tile (+ halo) that K4's bulk copies read past the last slot
+  for (int b = 0; b < 2; ++b) { L.soa[b][0] = take(cap * 16 + (kPairThreads + kPairHalo) * 16); L.soa[b][1] = take(cap * 2 + kPairThreads * 2); }
   L.off = take(cap * 4); L.disp = take(cap * 4); L.prop = take(cap * 4);
   L.best = take(cap * 8);
   L.hasprop = take((cap / 32 + 16) * 4);
@@ -428,7 +429,8 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     s->grid_move = sized(occ, (uint64_t)kMoveThreads * s->k1_unroll);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_scat, kMoveThreads, s->pack_disp ? 0 : gsm);
     s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * s->k3_unroll);
-    s->grid_pairs = (uint32_t)(((uint64_t)cfg->capacity + kPairThreads - 1) / kPairThreads);   // one tile per block
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pairs, kPairThreads, 0);
+    s->grid_pairs = sized(occ, kPairThreads);                  // persistent: tiles are dealt round-robin
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, kUniThreads, 0);
     s->grid_uni = sized(occ, kUniTile);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_resolve, 256, 0);
