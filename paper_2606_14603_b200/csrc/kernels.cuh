@@ -405,39 +405,42 @@ __device__ __forceinline__ void delta_flush(const int32_t* s_delta, uint32_t* __
 // the rest of the agent's own cell, the +x cell, and the overlapped cells of the rows (y+1, z) and
 // (y-1..y+1, z+1).  With x-fastest cell keys the cells of one (y,z) row are one contiguous slot range.
 //
-// Work layout (round 2; profiles/r2_pairs.md has the per-phase instruction split that led here: set-up,
-// divergent row visits and one-lane hit qualification were 70 % of the instructions, and a first cut with
-// per-tile block queues was bound by the barrier before the rare work).  The kernel is persistent: a
-// block walks tiles of 256 consecutive sorted slots; the records of the NEXT tile (plus kPairHalo slots
-// behind it) and its species arrive in shared memory by two bulk copies (cp.async.bulk + mbarrier, the
-// TMA engine) while the current tile is worked on, so no warp ever waits on the streaming loads.
-// Per tile every warp does dense work only:
+// Work layout (round 2; profiles/r2_pairs.md has the per-phase instruction split and the two discarded
+// cuts that led here: set-up, divergent row visits and one-lane hit qualification were 70 % of the
+// instructions of the round-1 kernel, and block-wide queues drained behind block barriers were latency-bound).
+// The kernel is persistent and its warps run on their own.  A block walks tiles of 256 consecutive sorted
+// slots; tile records (plus kPairHalo slots behind them) and species arrive in a four-stage shared-memory
+// ring by bulk copies (cp.async.bulk + mbarrier: the TMA engine) issued by a ninth, producer warp up to three
+// tiles ahead of the tile being worked on, so no warp waits on the streaming loads; a stage is handed back by one mbarrier arrival per warp, so
+// there is no block-wide barrier in the loop.  Per tile a warp owns 32 slots and does dense work only:
 //  A  own row.  Every agent tests the kPairWin slots behind its own straight from shared memory: no
 //     range look-up, no loop, every lane busy.  A slot that passes the window test (|d| <= R on every
 //     axis) is a genuine close pair whatever cell it lies in, so nothing has to bound the window; the
 //     own-row range (rest of the own cell, plus the +x cell if the R-ball reaches it) is longer than
 //     the window only if the slot right behind the window still lies in that x interval: then the
-//     remainder becomes a task.
-//  B  agents that face a +y / +z cell (about a fifth) append one 8-byte task per forward row (owner
-//     slot, first cell of the range, cells in it) to the block's task queue; window hits go to the block's hit
-//     queue as (i, j, id_j, d2).
-// The rare work is DEFERRED until a block's worth of it has piled up (every few tiles), so that it too runs
-// with every lane busy and its look-up latency is paid once per batch instead of once per tile:
-//  C  task drain: one thread per task: two cell-range look-ups, then records in groups of four.
-//  D  hit drain: one thread per hit: reaction look-up, exact radius, symmetric pair draw and, if the pair
+//     remainder is row code 4 of the agent's entry.
+//  B  agents with rows to visit (a +y / +z cell face within R, or a remainder: about a fifth) append one
+//     entry (slot, row mask) to the WARP's queue: one ballot, no atomics.  Window hits go to the warp's
+//     hit queue as (i, j, id_j, d2).
+// The rare work is deferred until a warp's worth has piled up, so that it too runs with every lane busy,
+// and while one warp waits on its look-ups the others carry on with their tiles:
+//  C  32 entries: one lane per entry re-derives the agent's place in the grid and walks its rows (two
+//     cell-range look-ups, then records in groups of four).
+//  D  hits: one lane per hit: reaction look-up, exact radius, symmetric pair draw and, if the pair
 //     qualifies, the two atomic mins.  best[] is touched only there (rare), so it costs no bandwidth;
 //     hasprop gets one bit per touched agent and prop[] the slot of a partner that qualified.  prop[] is a
 //     plain store (no round trip for the old key): with several qualifying partners it may name another than the
 //     minimum, so K4b checks id[prop[i]] against the key and searches the neighbourhood again in that
 //     (rare) case.  A pair reached twice (window and row) is merged twice, which changes nothing.
-// The task queue holds a drain mark's worth plus a whole tile (at most five tasks per agent), so it cannot
-// overflow; a hit that finds its queue full (dense test inputs) is qualified on the spot by the thread that found it.
+// The entry queue cannot overflow (fewer than 32 entries before a tile, at most 32 more); a hit that finds
+// its queue full (dense test inputs) is qualified on the spot.
 constexpr int kPairThreads = 256;
+constexpr int kPairWarps = kPairThreads / 32;
+constexpr int kPairStages = 4;
+constexpr int kPairBlock = kPairThreads + 32;   // 8 warps that own 32 slots of the tile each + the producer warp
 constexpr int kPairWin = 8;             // slots behind its own that every agent tests in phase A
 constexpr int kPairHalo = 16;           // slots staged behind the tile: kPairWin + the over-run probe, rounded up
-constexpr int kPairTaskDrain = 256;                        // a block's worth of tasks: drain before the next tile
-constexpr int kPairTaskCap = kPairTaskDrain + 5 * kPairThreads;   // ... so a tile (<= 5 tasks per agent) always fits
-constexpr int kPairHitCap = 128, kPairHitDrain = 64;
+constexpr int kPairHitCap = 32, kPairHitDrain = 16;    // per warp
 constexpr uint32_t kPairTileBytes = (kPairThreads + kPairHalo) * 16u + kPairThreads * 2u;
 constexpr unsigned long long kNoKey = ~0ull;
 
@@ -448,6 +451,9 @@ __device__ __forceinline__ void mbar_init(unsigned long long* bar, uint32_t coun
 }
 __device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
 }
 __device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, uint32_t parity) {
   uint32_t ok;
@@ -461,12 +467,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 struct PairSmem {
-  int4 rec[2][kPairThreads + kPairHalo];   // x, y, z, id of the tile's slots and the kPairHalo behind them
-  uint16_t sp[2][kPairThreads];            // species
-  uint2 task[kPairTaskCap];                // owner slot, first cell | (cells - 1) << 30   (3: own-row remainder)
-  uint4 hit[kPairHitCap];                  // i, j, id_j, d2
-  unsigned long long bar[2];
-  uint32_t ntask, nhit;
+  int4 rec[kPairStages][kPairThreads + kPairHalo];   // x, y, z, id of the tile's slots and the kPairHalo behind them
+  uint16_t sp[kPairStages][kPairThreads];            // species
+  uint4 hit[kPairWarps][kPairHitCap];                // i, j, id_j, d2
+  uint2 entry[kPairWarps][64];                       // slot, row mask
+  unsigned long long full[kPairStages], empty[kPairStages];
+  uint32_t nhit[kPairWarps];
 };
 
 // Reaction look-up, exact radius and symmetric pair draw for the geometric hit (i, j); on success both ends are merged.
@@ -486,23 +492,20 @@ __device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t
   atomicOr(&p.hasprop[i >> 5], 1u << (i & 31u));
   atomicOr(&p.hasprop[j >> 5], 1u << (j & 31u));
 }
-
 __device__ __noinline__ void pair_merge_now(const Params* p, uint32_t i, uint32_t j, uint32_t idj, uint32_t d2) {
   pair_merge(*p, i, j, idj, d2);
 }
-// Returns true when the hit queue has reached its drain mark.  A hit that finds the queue full (dense test
-// inputs) is qualified on the spot.
-__device__ __forceinline__ bool push_hit(const Params& p, PairSmem& S, uint32_t i, uint32_t j, uint32_t idj, uint32_t d2) {
-  const uint32_t h = atomicAdd(&S.nhit, 1u);
-  if (h < (uint32_t)kPairHitCap) S.hit[h] = make_uint4(i, j, idj, d2);
+// A hit that finds the warp's queue full (dense test inputs) is qualified on the spot.
+__device__ __forceinline__ void push_hit(const Params& p, PairSmem& S, uint32_t warp, uint32_t i, uint32_t j, uint32_t idj,
+                                         uint32_t d2) {
+  const uint32_t h = atomicAdd(&S.nhit[warp], 1u);
+  if (h < (uint32_t)kPairHitCap) S.hit[warp][h] = make_uint4(i, j, idj, d2);
   else pair_merge_now(&p, i, j, idj, d2);
-  return h + 1u >= (uint32_t)kPairHitDrain;
 }
 
 // Global slots [j0, j1) against agent i at (x, y, z).
-__device__ __forceinline__ bool scan_rows(const Params& p, PairSmem& S, uint32_t j0, uint32_t j1, uint32_t n,
+__device__ __forceinline__ void scan_rows(const Params& p, PairSmem& S, uint32_t warp, uint32_t j0, uint32_t j1, uint32_t n,
                                           uint32_t i, int32_t x, int32_t y, int32_t z) {
-  bool full = false;
   const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
   const int32_t ox = R - x, oy = R - y, oz = R - z;
@@ -523,127 +526,148 @@ __device__ __forceinline__ bool scan_rows(const Params& p, PairSmem& S, uint32_t
       const int4 q = __ldg(Rr + jj);
       const int32_t dx = q.x - x, dy = q.y - y, dz = q.z - z;     // each within +-R
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (jj < n && d2 <= p.max_r2) full |= push_hit(p, S, i, jj, (uint32_t)q.w, d2);
+      if (jj < n && d2 <= p.max_r2) push_hit(p, S, warp, i, jj, (uint32_t)q.w, d2);
     }
   }
-  return full;
 }
 
-__device__ __forceinline__ void pair_issue_tile(const Params& p, PairSmem& S, uint32_t buf, uint32_t tile) {
-  // generic-proxy reads of this buffer (two tiles ago) are ordered before the async-proxy refill
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-  mbar_expect_tx(&S.bar[buf], kPairTileBytes);
-  bulk_g2s(S.rec[buf], p.oth.r + (size_t)tile * kPairThreads, (kPairThreads + kPairHalo) * 16u, &S.bar[buf]);
-  bulk_g2s(S.sp[buf], p.oth.sp + (size_t)tile * kPairThreads, kPairThreads * 2u, &S.bar[buf]);
+// Where an agent sits in the cell grid: its own cell (linear index), whether its R-ball reaches the -x / +x
+// neighbour, and the forward rows it faces: bit (dz+1)*3 + (dy+1): (y+1, z) = 5; (y-1, z+1), (y, z+1),
+// (y+1, z+1) = 6, 7, 8.  R <= cell_size (validated), so the ball reaches at most one cell further on each side.
+struct PairGeo { uint32_t cell, xm, xp, rows; int32_t xlo; };
+__device__ __forceinline__ PairGeo pair_geo(const Params& p, int32_t x, int32_t y, int32_t z) {
+  const int32_t R = p.max_r, cs = p.cell_size;
+  const int32_t cx = cell_coord(x, p), cy = cell_coord(y, p), cz = cell_coord(z, p);
+  const int32_t lx = x - cx * cs, ly = y - cy * cs, lz = z - cz * cs;
+  PairGeo g;
+  g.xlo = x - lx;
+  g.xm = lx < R && cx > 0; g.xp = lx >= cs - R && cx < p.nx - 1;
+  const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
+  const uint32_t zp = lz >= cs - R && cz < p.nz - 1;
+  g.cell = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx + (uint32_t)cx;
+  g.rows = (yp << 5) | (zp ? ((ym | 2u | (yp << 2)) << 6) : 0u);
+  return g;
 }
 
-// C / D: drain the block's queues (called by every thread of the block).  Nobody appends tasks in here, and hits
-// are appended only before the first barrier, so the counters read below are the same for every thread.
-// Kept out of line: its registers (Philox, 64-bit keys) must not be charged to the dense per-tile loop.
-__device__ __noinline__ void pair_drain(const Params* pp, PairSmem* Sp, uint32_t n, bool all) {
+// C / D for one warp: entries [e0, e1) of its queue (one lane each), then its hits if `hits_too`.  Out of line:
+// its registers (Philox, 64-bit keys) must not be charged to the dense per-tile loop.
+__device__ __noinline__ void pair_drain(const Params* pp, PairSmem* Sp, uint32_t n, uint32_t e0, uint32_t e1, bool hits_too) {
   const Params& p = *pp;
   PairSmem& S = *Sp;
-  const uint32_t nt = S.ntask;
-  const bool dt = all || nt >= (uint32_t)kPairTaskDrain;
-  if (dt) {
-    for (uint32_t k = threadIdx.x; k < nt; k += kPairThreads) {     // one thread per task
-      const uint2 tk = S.task[k];
-      const int4 o = __ldg(p.oth.r + tk.x);
-      const uint32_t c0 = tk.y & 0x3FFFFFFFu, nc = tk.y >> 30;    // first cell | (cells - 1) << 30, or own-row remainder
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  __syncwarp();
+  if (e0 + lane < e1) {
+    const uint2 en = S.entry[warp][e0 + lane];
+    const uint32_t i = en.x;
+    const int4 o = __ldg(p.oth.r + i);
+    const PairGeo g = pair_geo(p, o.x, o.y, o.z);
+    uint32_t m = en.y;
+    while (m) {
+      const uint32_t c = __ffs(m) - 1u;
+      m &= m - 1u;
       uint32_t j0, j1;
-      if (nc == 3u) { j0 = tk.x + 1u + (uint32_t)kPairWin; j1 = p.cell[c0 + 1u]; }    // c0 = last cell of the own-row range
-      else { j0 = p.cell[c0]; j1 = p.cell[c0 + nc + 1u]; }
-      scan_rows(p, S, j0, j1, n, tk.x, o.x, o.y, o.z);
+      if (c == 4u) { j0 = i + 1u + (uint32_t)kPairWin; j1 = p.cell[g.cell + g.xp + 1u]; }       // own-row remainder
+      else {
+        const uint32_t c0 = g.cell + (uint32_t)p.fwd_row[c - 5u];      // host-precomputed row offsets of codes 5..8
+        j0 = p.cell[c0 - g.xm]; j1 = p.cell[c0 + g.xp + 1u];
+      }
+      scan_rows(p, S, warp, j0, j1, n, i, o.x, o.y, o.z);
     }
   }
-  __syncthreads();
-  const uint32_t nh = min(S.nhit, (uint32_t)kPairHitCap);
-  const bool dh = all || nh >= (uint32_t)kPairHitDrain;
-  if (dh) {
-    for (uint32_t h = threadIdx.x; h < nh; h += kPairThreads) {     // one thread per hit
-      const uint4 e = S.hit[h];
+  __syncwarp();
+  if (hits_too) {
+    const uint32_t nh = min(S.nhit[warp], (uint32_t)kPairHitCap);
+    if (lane < nh) {
+      const uint4 e = S.hit[warp][lane];
       pair_merge(p, e.x, e.y, e.z, e.w);
     }
+    __syncwarp();
+    if (lane == 0) S.nhit[warp] = 0;
+    __syncwarp();
   }
-  __syncthreads();
-  if (threadIdx.x == 0) { if (dt) S.ntask = 0; if (dh) S.nhit = 0; }
-  __syncthreads();
 }
 
-__global__ void __launch_bounds__(kPairThreads, 4) k_pairs(const __grid_constant__ Params p) {
+__device__ __forceinline__ void pair_issue_tile(const Params& p, PairSmem& S, uint32_t stage, uint32_t tile) {
+  // generic-proxy reads of this stage (by the tile that used it before) are ordered before the async-proxy refill
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  mbar_expect_tx(&S.full[stage], kPairTileBytes);
+  bulk_g2s(S.rec[stage], p.oth.r + (size_t)tile * kPairThreads, (kPairThreads + kPairHalo) * 16u, &S.full[stage]);
+  bulk_g2s(S.sp[stage], p.oth.sp + (size_t)tile * kPairThreads, kPairThreads * 2u, &S.full[stage]);
+}
+
+__global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__ Params p) {
   __shared__ __align__(128) PairSmem S;
   const uint32_t n = p.cell[p.n_cells];
   const uint32_t ntiles = (n + kPairThreads - 1u) / kPairThreads;
   if (blockIdx.x >= ntiles) return;
-  const uint32_t tid = threadIdx.x;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   if (tid == 0) {
-    S.ntask = 0; S.nhit = 0;
-    mbar_init(&S.bar[0], 1u); mbar_init(&S.bar[1], 1u);
+    for (int k = 0; k < kPairStages; ++k) { mbar_init(&S.full[k], 1u); mbar_init(&S.empty[k], (uint32_t)kPairWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    pair_issue_tile(p, S, 0u, blockIdx.x);
   }
-  __syncthreads();
-  const int32_t R = p.max_r, cs = p.cell_size;
+  if (lane == 0 && warp < (uint32_t)kPairWarps) S.nhit[warp] = 0;
+  __syncthreads();                  // the only block-wide barrier
+  if (warp == (uint32_t)kPairWarps) {
+    // ---- producer: keeps the ring full.  Tile `it` goes to stage it % kPairStages once every warp has handed back
+    // the tile that used it before.
+    if (lane == 0) {
+      uint32_t it = 0;
+      for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+        const uint32_t stage = it % (uint32_t)kPairStages, use = it / (uint32_t)kPairStages;
+        if (use) while (!mbar_try_wait(&S.empty[stage], (use - 1u) & 1u)) {}
+        pair_issue_tile(p, S, stage, tile);
+      }
+    }
+    return;
+  }
+  const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
-  uint32_t it = 0;
-  bool drain = false;        // block-uniform: a queue reached its drain mark during the previous tile
-  for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-    const uint32_t buf = it & 1u;
-    // ---- C / D: drain the queues once a block's worth has piled up
-    if (drain) pair_drain(&p, &S, n, false);
-    // next tile -> the other buffer (its readers finished before the barrier that ended the previous tile)
-    if (tid == 0 && tile + gridDim.x < ntiles) pair_issue_tile(p, S, buf ^ 1u, tile + gridDim.x);
-    while (!mbar_try_wait(&S.bar[buf], (it >> 1) & 1u)) {}
+  uint32_t nent = 0;                // entries in this warp's queue (warp-uniform)
+  uint32_t stage = 0, use = 0;      // tile `it` of this block: stage = it % kPairStages, use = it / kPairStages
+  for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    while (!mbar_try_wait(&S.full[stage], use & 1u)) {}
     const uint32_t i = tile * kPairThreads + tid;
-    const int4 q = S.rec[buf][tid];
-    const uint32_t s = S.sp[buf][tid];
-    bool want = false;       // this thread saw a queue reach its drain mark
+    const int4 q = S.rec[stage][tid];
+    const uint32_t s = S.sp[stage][tid];
+    uint32_t rows = 0;
     if (i < n && s != kDead && ((p.binds_mask >> s) & 1ull)) {
-      // where the agent sits in the cell grid.  R <= cell_size (validated), so its R-ball reaches at most one cell
-      // further on each side
-      const int32_t cx = cell_coord(q.x, p), cy = cell_coord(q.y, p), cz = cell_coord(q.z, p);
-      const int32_t lx = q.x - cx * cs, ly = q.y - cy * cs, lz = q.z - cz * cs;
-      const uint32_t xm = lx < R && cx > 0, xp = lx >= cs - R && cx < p.nx - 1;
-      const uint32_t ym = ly < R && cy > 0, yp = ly >= cs - R && cy < p.ny - 1;
-      const uint32_t zp = lz >= cs - R && cz < p.nz - 1;
-      // forward rows, bit (dz+1)*3 + (dy+1): (y+1, z) = 5; (y-1, z+1), (y, z+1), (y+1, z+1) = 6, 7, 8; 4 = own-row remainder
-      uint32_t rows = (yp << 5) | (zp ? ((ym | 2u | (yp << 2)) << 6) : 0u);
+      const PairGeo g = pair_geo(p, q.x, q.y, q.z);
+      rows = g.rows;
       // ---- A: the kPairWin slots behind its own
       const int32_t ox = R - q.x, oy = R - q.y, oz = R - q.z;
       uint32_t hits = 0;
 #pragma unroll
       for (uint32_t u = 0; u < (uint32_t)kPairWin; ++u) {
-        const int4 c = S.rec[buf][tid + 1u + u];
+        const int4 c = S.rec[stage][tid + 1u + u];
         const uint32_t ux = (uint32_t)(c.x + ox), uy = (uint32_t)(c.y + oy), uz = (uint32_t)(c.z + oz);
         hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;
       }
       for (; hits; hits &= hits - 1u) {                    // rare
         const uint32_t u = (uint32_t)__ffs(hits);
-        const int4 c = S.rec[buf][tid + u];
+        const int4 c = S.rec[stage][tid + u];
         const int32_t dx = c.x - q.x, dy = c.y - q.y, dz = c.z - q.z;
         const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-        if (i + u < n && d2 <= p.max_r2) want |= push_hit(p, S, i, i + u, (uint32_t)c.w, d2);   // never a slot past the population
+        if (i + u < n && d2 <= p.max_r2) push_hit(p, S, warp, i, i + u, (uint32_t)c.w, d2);   // never a slot past the population
       }
       // the own-row range goes on behind the window iff the next slot still lies in its x interval (slots of a row
       // are ordered by x cell; a slot of a LATER row that happens to lie in the interval only costs a look-up)
-      if ((uint32_t)(S.rec[buf][tid + 1u + kPairWin].x - cx * cs) < (1u + xp) * (uint32_t)cs) rows |= 1u << 4;
-      // ---- B: one task per row to visit (order is irrelevant: every hit is merged by atomic min)
-      if (rows) {
-        const uint32_t c0 = ((uint32_t)cz * (uint32_t)p.ny + (uint32_t)cy) * (uint32_t)p.nx + (uint32_t)cx;   // own cell
-        const uint32_t fv = (c0 - xm) | ((xm + xp) << 30);         // cells cx - xm .. cx + xp of a forward row
-        uint32_t pos = atomicAdd(&S.ntask, (uint32_t)__popc(rows));   // < kPairTaskDrain before the tile: a tile always fits
-        if (rows & 16u) S.task[pos++] = make_uint2(i, (c0 + xp) | (3u << 30));
-        if (rows & 32u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[0]);
-        if (rows & 64u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[1]);
-        if (rows & 128u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[2]);
-        if (rows & 256u) S.task[pos++] = make_uint2(i, fv + (uint32_t)p.fwd_row[3]);
-        want |= pos >= (uint32_t)kPairTaskDrain;
-      }
+      if ((uint32_t)(S.rec[stage][tid + 1u + kPairWin].x - g.xlo) < (1u + g.xp) * (uint32_t)p.cell_size) rows |= 1u << 4;
     }
-    // rec[buf] may be refilled, the queue counters are final for this tile, and every thread learns whether to drain
-    drain = __syncthreads_or(want);
+    // ---- B: one entry per agent with rows to visit, appended to the warp's queue
+    const uint32_t any = __ballot_sync(0xFFFFFFFFu, rows != 0u);
+    if (rows) S.entry[warp][nent + (uint32_t)__popc(any & ((1u << lane) - 1u))] = make_uint2(i, rows);
+    nent += (uint32_t)__popc(any);
+    // this warp is done with the stage
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&S.empty[stage]);
+    // ---- C / D once a warp's worth has piled up (hits ride along when there are enough of them)
+    if (nent >= 32u) {
+      nent -= 32u;
+      pair_drain(&p, &S, n, nent, nent + 32u, S.nhit[warp] >= (uint32_t)kPairHitDrain);
+    }
+    if (++stage == (uint32_t)kPairStages) { stage = 0; ++use; }
   }
-  pair_drain(&p, &S, n, true);
+  pair_drain(&p, &S, n, 0u, nent, true);
 }
 
 // ----------------------------------------------------------------------------- K4b handshake resolve

@@ -232,7 +232,7 @@ int enqueue_step(sim* s) {
     k_cell_scan<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_SCATTER);
     s->k_scat<<<s->grid_scatter, kMoveThreads, (s->gauss_in_smem && !s->pack_disp) ? s->gauss_bytes : 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairThreads, 0, s->run>>>(p); }
+  { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairBlock, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_BIRTHS); k_births<<<s->tail_blocks, kScanThreads, 0, s->run>>>(p); }
@@ -429,7 +429,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     s->grid_move = sized(occ, (uint64_t)kMoveThreads * s->k1_unroll);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_scat, kMoveThreads, s->pack_disp ? 0 : gsm);
     s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * s->k3_unroll);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pairs, kPairThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pairs, kPairBlock, 0);
     s->grid_pairs = sized(occ, kPairThreads);                  // persistent: tiles are dealt round-robin
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, kUniThreads, 0);
     s->grid_uni = sized(occ, kUniTile);
