@@ -96,6 +96,8 @@ struct Params {
   uint32_t n_cells;
   int32_t max_r;            // max interaction radius (ceil sqrt of max r2)
   uint32_t max_r2;
+  uint32_t pack_shift, pack_k1, pack_u;   // K4's packed window test: coordinate shift, T + 2^w and 2^w - 1 - 2T per field
+  uint32_t pack_span1, pack_span2;       // one / two cells in coarse x units (clamped to the field)
   uint32_t row_width;       // n_replicas * n_species
   unsigned long long binds_mask;   // bit s: species s takes part in a bimolecular reaction
   unsigned long long chan_mask;    // bit s: species s has unimolecular channels

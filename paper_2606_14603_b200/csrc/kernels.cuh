@@ -471,6 +471,7 @@ struct PairSmem {
   uint16_t sp[kPairStages][kPairThreads];            // species
   uint4 hit[kPairWarps][kPairHitCap];                // i, j, id_j, d2
   uint2 entry[kPairWarps][64];                       // slot, row mask
+  uint32_t key[kPairWarps][48];                      // packed coarse positions of the warp's 32 slots + the window behind
   unsigned long long full[kPairStages], empty[kPairStages];
   uint32_t nhit[kPairWarps];
 };
@@ -529,6 +530,22 @@ __device__ __forceinline__ void scan_rows(const Params& p, PairSmem& S, uint32_t
       if (jj < n && d2 <= p.max_r2) push_hit(p, S, warp, i, jj, (uint32_t)q.w, d2);
     }
   }
+}
+
+// Packed coarse position for the window test.  The LSU data pipe (shared-memory wavefronts), not instruction
+// issue, bounds this kernel (profiles/r2_pairs.md), and a 128-bit record per candidate costs four wavefronts per
+// warp; a 32-bit key costs one.  Key = three fields (x: 10 bits, y and z: 8 bits of the coordinate >> pack_shift,
+// i.e. modulo a few cells) with two guard bits above each, the lower guard set.  For keys a, b the sum
+// b + (K1 - a), K1 = T + 2^w per field, holds (b_f - a_f + T) mod 2^w in the low w bits of every field without
+// any carry between fields; adding U = 2^w - 1 - 2T per field to those low bits sets the guard iff the field
+// exceeds 2T.  T = ceil(R / 2^pack_shift), so |d| <= R on an axis implies a coarse difference within +-T
+// (modulo the field): the test never misses a pair; it passes about a third more candidates than the exact
+// window, and everything it passes is checked with the full coordinates afterwards.
+constexpr uint32_t kKeyLow = 0x3FFu | (0xFFu << 12) | (0xFFu << 22);
+constexpr uint32_t kKeyGuard = (1u << 10) | (1u << 20) | (1u << 30);
+__device__ __forceinline__ uint32_t pack_key(const Params& p, int32_t x, int32_t y, int32_t z) {
+  const uint32_t sh = p.pack_shift;
+  return (((uint32_t)x >> sh) & 0x3FFu) | ((((uint32_t)y >> sh) & 0xFFu) << 12) | ((((uint32_t)z >> sh) & 0xFFu) << 22) | kKeyGuard;
 }
 
 // Where an agent sits in the cell grid: its own cell (linear index), whether its R-ball reaches the -x / +x
@@ -620,8 +637,6 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
     }
     return;
   }
-  const int32_t R = p.max_r;
-  const uint32_t R2 = 2u * (uint32_t)R;
   uint32_t nent = 0;                // entries in this warp's queue (warp-uniform)
   uint32_t stage = 0, use = 0;      // tile `it` of this block: stage = it % kPairStages, use = it / kPairStages
   for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -629,29 +644,39 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
     const uint32_t i = tile * kPairThreads + tid;
     const int4 q = S.rec[stage][tid];
     const uint32_t s = S.sp[stage][tid];
+    // packed keys of the warp's 32 slots and of the kPairWin + 1 slots behind them (the first of the next warp's)
+    uint32_t* K = S.key[warp];
+    const uint32_t kq = pack_key(p, q.x, q.y, q.z);
+    K[lane] = kq;
+    if (lane <= (uint32_t)kPairWin) {
+      const int4 h = S.rec[stage][tid + 32u];
+      K[32u + lane] = pack_key(p, h.x, h.y, h.z);
+    }
+    __syncwarp();
     uint32_t rows = 0;
     if (i < n && s != kDead && ((p.binds_mask >> s) & 1ull)) {
       const PairGeo g = pair_geo(p, q.x, q.y, q.z);
       rows = g.rows;
       // ---- A: the kPairWin slots behind its own
-      const int32_t ox = R - q.x, oy = R - q.y, oz = R - q.z;
+      const uint32_t cq = p.pack_k1 - kq;
       uint32_t hits = 0;
 #pragma unroll
       for (uint32_t u = 0; u < (uint32_t)kPairWin; ++u) {
-        const int4 c = S.rec[stage][tid + 1u + u];
-        const uint32_t ux = (uint32_t)(c.x + ox), uy = (uint32_t)(c.y + oy), uz = (uint32_t)(c.z + oz);
-        hits |= (max(max(ux, uy), uz) <= R2) ? (1u << u) : 0u;
+        const uint32_t e = K[lane + 1u + u] + cq;
+        hits |= ((((e & kKeyLow) + p.pack_u) & kKeyGuard) == 0u) ? (1u << u) : 0u;
       }
-      for (; hits; hits &= hits - 1u) {                    // rare
+      for (; hits; hits &= hits - 1u) {                    // rare: the exact test
         const uint32_t u = (uint32_t)__ffs(hits);
         const int4 c = S.rec[stage][tid + u];
-        const int32_t dx = c.x - q.x, dy = c.y - q.y, dz = c.z - q.z;
-        const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-        if (i + u < n && d2 <= p.max_r2) push_hit(p, S, warp, i, i + u, (uint32_t)c.w, d2);   // never a slot past the population
+        const long long dx = (long long)c.x - q.x, dy = (long long)c.y - q.y, dz = (long long)c.z - q.z;
+        const unsigned long long d2 = (unsigned long long)(dx * dx + dy * dy + dz * dz);
+        if (i + u < n && d2 <= p.max_r2) push_hit(p, S, warp, i, i + u, (uint32_t)c.w, (uint32_t)d2);   // never a slot past the population
       }
       // the own-row range goes on behind the window iff the next slot still lies in its x interval (slots of a row
-      // are ordered by x cell; a slot of a LATER row that happens to lie in the interval only costs a look-up)
-      if ((uint32_t)(S.rec[stage][tid + 1u + kPairWin].x - g.xlo) < (1u + g.xp) * (uint32_t)p.cell_size) rows |= 1u << 4;
+      // are ordered by x cell).  Tested on the coarse x, modulo the field: a slot that only seems to lie in the
+      // interval (another row, or an alias) costs a look-up, nothing else.
+      const uint32_t xk = (K[lane + 1u + kPairWin] - ((uint32_t)g.xlo >> p.pack_shift)) & 0x3FFu;
+      if (xk <= (g.xp ? p.pack_span2 : p.pack_span1)) rows |= 1u << 4;
     }
     // ---- B: one entry per agent with rows to visit, appended to the warp's queue
     const uint32_t any = __ballot_sync(0xFFFFFFFFu, rows != 0u);

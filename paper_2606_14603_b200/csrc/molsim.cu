@@ -391,6 +391,18 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   p.max_r = (int32_t)std::ceil(std::sqrt((double)max_r2));
   while ((uint64_t)p.max_r * p.max_r < max_r2) p.max_r++;
   p.row_width = cfg->n_replicas * cfg->n_species;
+  {
+    // packed window test of K4 (kernels.cuh, pack_key): T = ceil(R / 2^shift) <= 15 coarse units per axis
+    uint32_t sh = 0;
+    while ((((uint32_t)p.max_r + (1u << sh) - 1u) >> sh) > 15u) ++sh;
+    const uint32_t T = ((uint32_t)p.max_r + (1u << sh) - 1u) >> sh;
+    p.pack_shift = sh;
+    p.pack_k1 = (T + (1u << 10)) | ((T + (1u << 8)) << 12) | ((T + (1u << 8)) << 22);
+    p.pack_u = ((1u << 10) - 1u - 2u * T) | (((1u << 8) - 1u - 2u * T) << 12) | (((1u << 8) - 1u - 2u * T) << 22);
+    // a slot in the x interval [xlo, xlo + span) has a coarse x at most ((span - 1) >> shift) + 1 above xlo's
+    p.pack_span1 = std::min<uint32_t>(((cfg->cell_size - 1u) >> sh) + 1u, 1023u);
+    p.pack_span2 = std::min<uint32_t>(((2u * cfg->cell_size - 1u) >> sh) + 1u, 1023u);
+  }
   p.top_shift = 16;                                                   // birth_top: at most kMaxTop entries
   while ((((uint64_t)cfg->id_capacity - 1) >> p.top_shift) + 1 > kMaxTop) p.top_shift++;
 
