@@ -438,9 +438,9 @@ constexpr int kPairThreads = 256;
 constexpr int kPairWarps = kPairThreads / 32;
 constexpr int kPairStages = 4;
 constexpr int kPairBlock = kPairThreads + 32;   // 8 warps that own 32 slots of the tile each + the producer warp
-constexpr int kPairWin = 8;             // slots behind its own that every agent tests in phase A
+constexpr int kPairWin = 5;             // slots behind its own that every agent tests in phase A
 constexpr int kPairHalo = 16;           // slots staged behind the tile: kPairWin + the over-run probe, rounded up
-constexpr int kPairHitCap = 32, kPairHitDrain = 16;    // per warp
+constexpr int kPairHitCap = 16, kPairHitDrain = 8;     // per warp
 constexpr uint32_t kPairTileBytes = (kPairThreads + kPairHalo) * 16u + kPairThreads * 2u;
 constexpr unsigned long long kNoKey = ~0ull;
 
@@ -469,18 +469,22 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 struct PairSmem {
   int4 rec[kPairStages][kPairThreads + kPairHalo];   // x, y, z, id of the tile's slots and the kPairHalo behind them
   uint16_t sp[kPairStages][kPairThreads];            // species
-  uint4 hit[kPairWarps][kPairHitCap];                // i, j, id_j, d2
-  uint2 entry[kPairWarps][64];                       // slot, row mask
+  int4 ent_pos[kPairWarps][64];                      // per warp, agents with rows left to visit: x, y, z, id
+  uint4 ent_geo[kPairWarps][64];                     //   slot, own cell, rows | xm << 9 | xp << 10 | species << 16, -
+  uint4 hit_a[kPairWarps][kPairHitCap];              // per warp, window hits: i, j, id_i, id_j
+  uint2 hit_b[kPairWarps][kPairHitCap];              //   d2, species of i
   uint32_t key[kPairWarps][48];                      // packed coarse positions of the warp's 32 slots + the window behind
   unsigned long long full[kPairStages], empty[kPairStages];
   uint32_t nhit[kPairWarps];
 };
 
+__device__ __forceinline__ void prefetch_l1(const void* ptr) { asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr)); }
+
 // Reaction look-up, exact radius and symmetric pair draw for the geometric hit (i, j); on success both ends are merged.
-__device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t j, uint32_t idj, uint32_t d2) {
+__device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t j, uint32_t id, uint32_t idj, uint32_t d2,
+                                           uint32_t si) {
   const DevTables* __restrict__ T = p.tab;
-  const uint32_t si = p.oth.sp[i], sj = p.oth.sp[j], id = (uint32_t)p.oth.r[i].w;
-  const uint32_t e = T->rxmap[si * kMaxSpecies + sj];
+  const uint32_t e = T->rxmap[si * kMaxSpecies + p.oth.sp[j]];
   if (e == 0xFFu) return;
   const DevRx& rx = T->rx[e];
   if (d2 > rx.r2) return;
@@ -493,20 +497,26 @@ __device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t
   atomicOr(&p.hasprop[i >> 5], 1u << (i & 31u));
   atomicOr(&p.hasprop[j >> 5], 1u << (j & 31u));
 }
-__device__ __noinline__ void pair_merge_now(const Params* p, uint32_t i, uint32_t j, uint32_t idj, uint32_t d2) {
-  pair_merge(*p, i, j, idj, d2);
+__device__ __noinline__ void pair_merge_now(const Params* p, uint32_t i, uint32_t j, uint32_t id, uint32_t idj, uint32_t d2,
+                                            uint32_t si) {
+  pair_merge(*p, i, j, id, idj, d2, si);
 }
-// A hit that finds the warp's queue full (dense test inputs) is qualified on the spot.
-__device__ __forceinline__ void push_hit(const Params& p, PairSmem& S, uint32_t warp, uint32_t i, uint32_t j, uint32_t idj,
-                                         uint32_t d2) {
+// A hit that finds the warp's queue full (dense test inputs) is qualified on the spot.  The partner's species is the
+// one thing the drain will have to fetch: ask for its line now.
+__device__ __forceinline__ void push_hit(const Params& p, PairSmem& S, uint32_t warp, uint32_t i, uint32_t j, uint32_t id,
+                                         uint32_t idj, uint32_t d2, uint32_t si) {
   const uint32_t h = atomicAdd(&S.nhit[warp], 1u);
-  if (h < (uint32_t)kPairHitCap) S.hit[warp][h] = make_uint4(i, j, idj, d2);
-  else pair_merge_now(&p, i, j, idj, d2);
+  if (h < (uint32_t)kPairHitCap) {
+    S.hit_a[warp][h] = make_uint4(i, j, id, idj); S.hit_b[warp][h] = make_uint2(d2, si);
+    prefetch_l1(p.oth.sp + j);
+  } else {
+    pair_merge_now(&p, i, j, id, idj, d2, si);
+  }
 }
 
-// Global slots [j0, j1) against agent i at (x, y, z).
+// Global slots [j0, j1) against agent i (id, species si) at (x, y, z).
 __device__ __forceinline__ void scan_rows(const Params& p, PairSmem& S, uint32_t warp, uint32_t j0, uint32_t j1, uint32_t n,
-                                          uint32_t i, int32_t x, int32_t y, int32_t z) {
+                                          uint32_t i, uint32_t id, uint32_t si, int32_t x, int32_t y, int32_t z) {
   const int32_t R = p.max_r;
   const uint32_t R2 = 2u * (uint32_t)R;
   const int32_t ox = R - x, oy = R - y, oz = R - z;
@@ -527,7 +537,7 @@ __device__ __forceinline__ void scan_rows(const Params& p, PairSmem& S, uint32_t
       const int4 q = __ldg(Rr + jj);
       const int32_t dx = q.x - x, dy = q.y - y, dz = q.z - z;     // each within +-R
       const uint32_t d2 = (uint32_t)(dx * dx) + (uint32_t)(dy * dy) + (uint32_t)(dz * dz);
-      if (jj < n && d2 <= p.max_r2) push_hit(p, S, warp, i, jj, (uint32_t)q.w, d2);
+      if (jj < n && d2 <= p.max_r2) push_hit(p, S, warp, i, jj, id, (uint32_t)q.w, d2, si);
     }
   }
 }
@@ -566,42 +576,61 @@ __device__ __forceinline__ PairGeo pair_geo(const Params& p, int32_t x, int32_t 
   return g;
 }
 
-// C / D for one warp: entries [e0, e1) of its queue (one lane each), then its hits if `hits_too`.  Out of line:
-// its registers (Philox, 64-bit keys) must not be charged to the dense per-tile loop.
-__device__ __noinline__ void pair_drain(const Params* pp, PairSmem* Sp, uint32_t n, uint32_t e0, uint32_t e1, bool hits_too) {
+// Address of the first cell-range word the row with the lowest code in `rows` will look up.
+__device__ __forceinline__ const uint32_t* first_lookup(const Params& p, uint32_t cell, uint32_t rows, uint32_t xm, uint32_t xp) {
+  const uint32_t c = (uint32_t)__ffs(rows) - 1u;
+  return p.cell + (c == 4u ? cell + xp + 1u : cell + (uint32_t)p.fwd_row[c - 5u] - xm);
+}
+
+// C / D for one warp.  Takes up to 32 entries off the top of its queue and visits ONE row of each (two cell-range
+// look-ups, whose line was prefetched when the entry was queued, then records in groups of four); an entry with
+// further rows goes back on the queue, so every round is dense and costs one memory round trip.  Then, if there are
+// enough of them (or `all`), the warp's hits.  Returns the new queue length.  Out of line: its registers (Philox,
+// 64-bit keys) must not be charged to the dense per-tile loop.
+__device__ __noinline__ uint32_t pair_drain(const Params* pp, PairSmem* Sp, uint32_t n, uint32_t nent, bool all) {
   const Params& p = *pp;
   PairSmem& S = *Sp;
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   __syncwarp();
-  if (e0 + lane < e1) {
-    const uint2 en = S.entry[warp][e0 + lane];
-    const uint32_t i = en.x;
-    const int4 o = __ldg(p.oth.r + i);
-    const PairGeo g = pair_geo(p, o.x, o.y, o.z);
-    uint32_t m = en.y;
-    while (m) {
-      const uint32_t c = __ffs(m) - 1u;
-      m &= m - 1u;
-      uint32_t j0, j1;
-      if (c == 4u) { j0 = i + 1u + (uint32_t)kPairWin; j1 = p.cell[g.cell + g.xp + 1u]; }       // own-row remainder
-      else {
-        const uint32_t c0 = g.cell + (uint32_t)p.fwd_row[c - 5u];      // host-precomputed row offsets of codes 5..8
-        j0 = p.cell[c0 - g.xm]; j1 = p.cell[c0 + g.xp + 1u];
-      }
-      scan_rows(p, S, warp, j0, j1, n, i, o.x, o.y, o.z);
+  const uint32_t take = min(nent, 32u), e0 = nent - take;
+  int4 o = make_int4(0, 0, 0, 0);
+  uint4 ge = make_uint4(0, 0, 0, 0);
+  uint32_t left = 0;
+  if (lane < take) {
+    o = S.ent_pos[warp][e0 + lane]; ge = S.ent_geo[warp][e0 + lane];
+    const uint32_t rows = ge.z & 0x1F0u, xm = ge.z >> 9 & 1u, xp = ge.z >> 10 & 1u;
+    const uint32_t c = (uint32_t)__ffs(rows) - 1u;
+    left = rows & (rows - 1u);
+    uint32_t j0, j1;
+    if (c == 4u) { j0 = ge.x + 1u + (uint32_t)kPairWin; j1 = p.cell[ge.y + xp + 1u]; }       // own-row remainder
+    else {
+      const uint32_t c0 = ge.y + (uint32_t)p.fwd_row[c - 5u];      // host-precomputed row offsets of codes 5..8
+      j0 = p.cell[c0 - xm]; j1 = p.cell[c0 + xp + 1u];
     }
+    scan_rows(p, S, warp, j0, j1, n, ge.x, (uint32_t)o.w, ge.z >> 16, o.x, o.y, o.z);
   }
+  __syncwarp();            // every lane has read its entry: the slots may be overwritten
+  const uint32_t again = __ballot_sync(0xFFFFFFFFu, left != 0u);
+  if (left) {
+    const uint32_t k = e0 + (uint32_t)__popc(again & ((1u << lane) - 1u));
+    ge.z = (ge.z & ~0x1F0u) | left;
+    S.ent_pos[warp][k] = o; S.ent_geo[warp][k] = ge;
+    prefetch_l1(first_lookup(p, ge.y, left, ge.z >> 9 & 1u, ge.z >> 10 & 1u));
+  }
+  nent = e0 + (uint32_t)__popc(again);
   __syncwarp();
-  if (hits_too) {
-    const uint32_t nh = min(S.nhit[warp], (uint32_t)kPairHitCap);
+  const uint32_t nh = min(S.nhit[warp], (uint32_t)kPairHitCap);
+  if (nh >= (uint32_t)kPairHitDrain || (all && nh)) {
     if (lane < nh) {
-      const uint4 e = S.hit[warp][lane];
-      pair_merge(p, e.x, e.y, e.z, e.w);
+      const uint4 a = S.hit_a[warp][lane];
+      const uint2 b = S.hit_b[warp][lane];
+      pair_merge(p, a.x, a.y, a.z, a.w, b.x, b.y);
     }
     __syncwarp();
     if (lane == 0) S.nhit[warp] = 0;
     __syncwarp();
   }
+  return nent;
 }
 
 __device__ __forceinline__ void pair_issue_tile(const Params& p, PairSmem& S, uint32_t stage, uint32_t tile) {
@@ -631,7 +660,7 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
       uint32_t it = 0;
       for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
         const uint32_t stage = it % (uint32_t)kPairStages, use = it / (uint32_t)kPairStages;
-        if (use) while (!mbar_try_wait(&S.empty[stage], (use - 1u) & 1u)) {}
+        if (use) while (!mbar_try_wait(&S.empty[stage], (use - 1u) & 1u)) __nanosleep(256);   // do not spin on issue slots
         pair_issue_tile(p, S, stage, tile);
       }
     }
@@ -653,10 +682,10 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
       K[32u + lane] = pack_key(p, h.x, h.y, h.z);
     }
     __syncwarp();
-    uint32_t rows = 0;
+    uint32_t rows = 0, cell = 0;        // rows to visit | xm << 9 | xp << 10, own cell
     if (i < n && s != kDead && ((p.binds_mask >> s) & 1ull)) {
       const PairGeo g = pair_geo(p, q.x, q.y, q.z);
-      rows = g.rows;
+      rows = g.rows; cell = g.cell;
       // ---- A: the kPairWin slots behind its own
       const uint32_t cq = p.pack_k1 - kq;
       uint32_t hits = 0;
@@ -670,29 +699,34 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
         const int4 c = S.rec[stage][tid + u];
         const long long dx = (long long)c.x - q.x, dy = (long long)c.y - q.y, dz = (long long)c.z - q.z;
         const unsigned long long d2 = (unsigned long long)(dx * dx + dy * dy + dz * dz);
-        if (i + u < n && d2 <= p.max_r2) push_hit(p, S, warp, i, i + u, (uint32_t)c.w, (uint32_t)d2);   // never a slot past the population
+        if (i + u < n && d2 <= p.max_r2)                   // never a slot past the population
+          push_hit(p, S, warp, i, i + u, (uint32_t)q.w, (uint32_t)c.w, (uint32_t)d2, s);
       }
       // the own-row range goes on behind the window iff the next slot still lies in its x interval (slots of a row
       // are ordered by x cell).  Tested on the coarse x, modulo the field: a slot that only seems to lie in the
       // interval (another row, or an alias) costs a look-up, nothing else.
       const uint32_t xk = (K[lane + 1u + kPairWin] - ((uint32_t)g.xlo >> p.pack_shift)) & 0x3FFu;
       if (xk <= (g.xp ? p.pack_span2 : p.pack_span1)) rows |= 1u << 4;
+      if (rows) rows |= (g.xm << 9) | (g.xp << 10);
     }
-    // ---- B: one entry per agent with rows to visit, appended to the warp's queue
+    // ---- B: one entry per agent with rows to visit, appended to the warp's queue; the cell-range words its first row
+    // will look up are asked for now
     const uint32_t any = __ballot_sync(0xFFFFFFFFu, rows != 0u);
-    if (rows) S.entry[warp][nent + (uint32_t)__popc(any & ((1u << lane) - 1u))] = make_uint2(i, rows);
+    if (rows) {
+      const uint32_t k = nent + (uint32_t)__popc(any & ((1u << lane) - 1u));
+      S.ent_pos[warp][k] = q;
+      S.ent_geo[warp][k] = make_uint4(i, cell, rows | (s << 16), 0u);
+      prefetch_l1(first_lookup(p, cell, rows & 0x1F0u, rows >> 9 & 1u, rows >> 10 & 1u));
+    }
     nent += (uint32_t)__popc(any);
     // this warp is done with the stage
     __syncwarp();
     if (lane == 0) mbar_arrive(&S.empty[stage]);
     // ---- C / D once a warp's worth has piled up (hits ride along when there are enough of them)
-    if (nent >= 32u) {
-      nent -= 32u;
-      pair_drain(&p, &S, n, nent, nent + 32u, S.nhit[warp] >= (uint32_t)kPairHitDrain);
-    }
+    while (nent >= 32u) nent = pair_drain(&p, &S, n, nent, false);
     if (++stage == (uint32_t)kPairStages) { stage = 0; ++use; }
   }
-  pair_drain(&p, &S, n, 0u, nent, true);
+  do { nent = pair_drain(&p, &S, n, nent, true); } while (nent);
 }
 
 // ----------------------------------------------------------------------------- K4b handshake resolve
