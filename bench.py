@@ -123,13 +123,12 @@ def ledger_bytes_per_agent(kernel, c):
     """Algorithmic HBM bytes per live agent per launch: SURVEY.md §8(d) "Design B" column, kernel by
     kernel (DESIGN.md §5 maps each of our kernels to its row); c = cells per agent."""
     return {
-        "k_move_hist": 18 + 12 + 8 * c,          # K1: R soa, W xyz, cell count RMW
+        "k_uni_hist": 18 + 12 + 8 * c + 14 + 4,  # K1 (R soa, W xyz, cell count RMW) fused with K5 (resolve + unimolecular)
         "memset_cells": 0.0, "k_cell_reduce": 0.0,
         "k_cell_scan": 8 * c,                    # K2
         "k_scatter": 18 + 18 + 8 * c,            # K3: R soa, W soa, cell starts
         "k_pairs": 18 + 4 + 8 * c,               # K4: R soa, W proposal, cell starts
         "k_resolve": 0.0,
-        "k_uni": 14 + 4,                         # K5: resolve + unimolecular
         "k_births": 0.5,                         # K6: births only + id bitmap
     }.get(kernel, 0.0)
 
@@ -139,12 +138,11 @@ def moved_bytes_per_agent(kernel, c):
     §8(d) ledger where a pass was elided (move recomputed in K3, sparse proposals), larger where it keeps an
     extra array (off)."""
     return {
-        "k_move_hist": 18 + 4 + 8 * c,           # R soa, W off, cell count RMW (moved positions are not stored)
+        "k_uni_hist": 18 + 8 * c,                # R soa once for both jobs, cell count RMW (moved positions are not stored)
         "memset_cells": 4 * c, "k_cell_reduce": 4 * c, "k_cell_scan": 8 * c,
-        "k_scatter": 18 + 4 + 18 + 4 * c,        # R soa + off, W soa, R cell starts
+        "k_scatter": 18 + 18 + 8 * c,            # R soa, W soa, cell cursor RMW
         "k_pairs": 18 + 0.125 + 4 * c,           # R record + species, W 1 bit; R cell starts
         "k_resolve": 0.125,                      # R proposal bitmap
-        "k_uni": 2,                              # R species (id / position only where a channel exists)
     }.get(kernel, 0.0)
 
 

@@ -148,7 +148,7 @@ uint64_t sim_launch_count(const sim_t*);
  * the stream (slower; for bench.py's roofline leg, not for throughput numbers).
  * sim_kernel_times returns, for each of the SIM_N_KERNELS kernels, accumulated milliseconds and
  * launch counts since the last enable. */
-#define SIM_N_KERNELS 11
+#define SIM_N_KERNELS 10
 int sim_profile_enable(sim_t*, int on);
 int sim_kernel_times(sim_t*, float ms[SIM_N_KERNELS], uint32_t launches[SIM_N_KERNELS]);
 const char* sim_kernel_name(int k);

@@ -8,7 +8,7 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("MOLSIM_LIB") or os.path.join(HERE, "libmolsim.so")   # override: tuning builds
-N_KERNELS = 11
+N_KERNELS = 10
 E_INVAL, E_CAPACITY, E_IDSPACE, E_CUDA = -1, -2, -3, -4
 
 

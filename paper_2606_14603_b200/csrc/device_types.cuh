@@ -69,12 +69,12 @@ struct Soa {
 struct Params {
   Soa cur, oth;             // cur: state at step start (moved in place); oth: cell-sorted copy,
                             // on which bind / unimolecular / births act in place
-  uint32_t* off;            // within-cell rank from the histogram pass
-  uint32_t* disp;           // accepted displacement of this step, 3 x 10 bits + crossing flag (K1 -> K3)
   unsigned long long* best; // proposal key (dist^2 << 32 | partner id) per sorted slot, ~0 = none
   uint32_t* prop;           // slot of the partner that last lowered best[i] (checked against the key in K4b)
   uint32_t* hasprop;        // 1 bit per sorted slot: best[i] was touched this step (cleared by K5)
-  uint32_t* cell;           // [n_cells + 1]: counts, then exclusive starts; cell[n_cells] = n_sorted
+  uint32_t* cell;           // this step's cell array: cell[0] = 0, cell[k + 1] = count of cell k (histogram), then its first
+                            // slot (scan), then its end (scatter): from K4 on cell[k] = first slot of cell k, cell[n_cells] = n_sorted
+  uint32_t* cell_next;      // the next step's cell array (histogram taken by this step's K5 / K6); the two swap every step
   uint32_t* partial;        // scan partials
   uint32_t* bits;           // birth bitmap, 4 bits per id
   uint32_t* birth_mid;      // newborns of this step per block of 256 parent ids

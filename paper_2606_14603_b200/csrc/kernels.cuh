@@ -1,8 +1,8 @@
 // kernels.cuh — the hand-written sm_100a kernels of the molecule-agent step.
 // Product code (CUDA path).  Shares nothing with oracle/.
 //
-// One step = K1 move+hist -> K2 cell scan (2 launches) -> K3 move+scatter -> K4 pair search/proposal ->
-// K4b resolve -> K5 unimolecular -> K6 births (ranking + placement, 1 launch) -> K7 epilogue: 10 launches.
+// One step = K2 cell scan (2 launches) -> K3 move+scatter -> K4 pair search/proposal -> K4b resolve ->
+// K5 unimolecular + cell histogram of the NEXT step -> K6 births + epilogue: 7 launches.
 // Every decision is keyed by agent id (never by slot), so the nondeterministic slot order the
 // histogram atomics produce inside a cell cannot change any result.
 #pragma once
@@ -82,12 +82,13 @@ __device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* s_warp /*[9]
   return total;
 }
 
-// ----------------------------------------------------------------------------- K1 move + histogram
+// ----------------------------------------------------------------------------- phase 1: move
 // Phase 1 (Brownian move, boundary and compartment rule) is a pure function of
-// (species, position, id, t): move_agent() below.  K1 evaluates it only to get the cell key for the
-// histogram of the counting sort (a3) and stores nothing but the within-cell rank; K3 evaluates it
-// again while it scatters, so the moved positions are written once, at their sorted slot, and the
-// 12 B/agent write + re-read of an in-place move never happens (a second Philox is cheaper).
+// (species, position, id, t): move_agent() below.  It is evaluated twice per agent and step: by the histogram
+// pass, which only needs the cell key of the moved position (and runs at the END of the previous step, fused
+// with the unimolecular pass that streams the same agents: k_uni_hist), and by K3 while it scatters, so the
+// moved positions are written once, at their sorted slot, and the 12 B/agent write + re-read of an in-place
+// move never happens (a second Philox is cheaper).
 struct Moved { int32_t x, y, z; uint16_t s; };
 
 // What phase 1 needs of the tables, staged in shared memory next to the Gaussian tables so that
@@ -147,26 +148,12 @@ __device__ __forceinline__ const int16_t* stage_tables(const Params& p, MoveTabl
   return g;
 }
 
-// A block walks tiles of 256 x kK1Unroll agents; every thread keeps kK1Unroll agents in flight
-// (all loads issued before the first Philox, all histogram atomics before the first rank store) so
-// that HBM and L2-atomic latency overlap.  The histogram uses warp-aggregated atomics
-// (__match_any_sync on the cell key): agents arrive nearly cell-sorted from the previous step, so a
-// warp touches few distinct cells.
-#ifndef MOLSIM_MATCH_ANY
-#define MOLSIM_MATCH_ANY 0      // 1: aggregate with __match_any_sync (measured slower)
-#endif
-// Warp aggregation of the histogram atomics.  Agents arrive nearly cell-sorted from the previous
+// Warp aggregation of the counting sort's atomics.  Agents arrive nearly cell-sorted from the previous
 // step, so lanes with equal keys are almost always neighbours: a run of equal keys (one shuffle, one
 // ballot) is aggregated into one atomic by its first lane.  Equal keys that are not adjacent simply
 // issue separate atomics.  (__match_any_sync finds them all but runs on the slow ADU pipe: it was
-// the top stall of this kernel.)
+// the top stall of the histogram kernel when tried.)
 __device__ __forceinline__ void run_of_key(uint32_t key, uint32_t lane, int& leader, uint32_t& rank, uint32_t& count) {
-#if MOLSIM_MATCH_ANY
-  const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
-  leader = __ffs(peers) - 1;
-  rank = __popc(peers & ((1u << lane) - 1u));
-  count = __popc(peers);
-#else
   const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, key, 1);
   const uint32_t heads = __ballot_sync(0xFFFFFFFFu, lane == 0u || key != prev);
   const uint32_t upto = (2u << lane) - 1u;                        // lanes 0..lane (lane 31: all ones)
@@ -175,81 +162,12 @@ __device__ __forceinline__ void run_of_key(uint32_t key, uint32_t lane, int& lea
   const int end = above ? __ffs(above) - 1 : 32;
   rank = lane - (uint32_t)leader;
   count = (uint32_t)(end - leader);
-#endif
 }
 
-// Agents in flight per thread (kU) and resident blocks per SM (kB) are template parameters of K1 and
-// K3; the host picks per problem size (swept on B200: profiles/r1e_kernels.md).  With the 16-byte records
-// K1 likes 4 agents per thread x 4 blocks/SM from a few million agents on; K3 keeps 2 x 5 at every size.
-struct MoveCfgSmall { static constexpr int k1u = 2, k1b = 5, k3u = 2, k3b = 5; };
-#ifndef MOLSIM_L_K1U      // tuning builds override the large-population shape
-#define MOLSIM_L_K1U 4
-#define MOLSIM_L_K1B 4
-#define MOLSIM_L_K3U 2
-#define MOLSIM_L_K3B 5
-#endif
-struct MoveCfgLarge { static constexpr int k1u = MOLSIM_L_K1U, k1b = MOLSIM_L_K1B, k3u = MOLSIM_L_K3U, k3b = MOLSIM_L_K3B; };
-constexpr uint32_t kLargeFrom = 2000000;   // capacity (agents) from which MoveCfgLarge is used
+// Agents in flight per thread and resident blocks per SM of the two passes that evaluate the move are
+// template parameters; the host picks per problem size (swept on B200: profiles/).
+constexpr uint32_t kLargeFrom = 2000000;   // capacity (agents) from which the large-population shapes are used
 constexpr int kMoveThreads = 256;
-
-// kPack: the accepted displacement (|d| <= 511 on every axis: validated by the host from the tables) and the
-// membrane-crossing flag are also written, packed into one 32-bit word per agent, so that K3 re-applies the move
-// with three adds instead of a second Philox + table + boundary evaluation.  Used while the state is
-// L2-resident (small populations); at 16 M agents the extra 4 B/agent stream costs more than the arithmetic.
-__device__ __forceinline__ uint32_t pack_disp(int32_t dx, int32_t dy, int32_t dz, bool crossed) {
-  return ((uint32_t)dx & 0x3FFu) | (((uint32_t)dy & 0x3FFu) << 10) | (((uint32_t)dz & 0x3FFu) << 20) | ((uint32_t)crossed << 30);
-}
-__device__ __forceinline__ int32_t unpack10(uint32_t w, uint32_t shift) { return (int32_t)(w << (22u - shift)) >> 22; }
-
-template <bool kGaussSmem, int kK1Unroll, int kMinBlk, bool kPack>
-__global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_move_hist(Params p) {
-  extern __shared__ __align__(16) int16_t s_gauss[];
-  __shared__ MoveTables M;
-  const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
-  const uint32_t n = p.scal->n_slots, t = p.scal->t;
-  const uint32_t lane = threadIdx.x & 31u;
-  constexpr uint32_t kTile = kMoveThreads * kK1Unroll;
-  for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {   // block-uniform trip count
-    uint16_t s[kK1Unroll];
-    int32_t x[kK1Unroll], y[kK1Unroll], z[kK1Unroll];
-    uint32_t id[kK1Unroll], key[kK1Unroll], dsp[kK1Unroll];
-#pragma unroll
-    for (int a = 0; a < kK1Unroll; ++a) {
-      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
-      s[a] = i < n ? p.cur.sp[i] : kDead;
-    }
-#pragma unroll
-    for (int a = 0; a < kK1Unroll; ++a) {
-      const uint32_t i = base + a * kMoveThreads + threadIdx.x;
-      if (i < n) { const int4 q = p.cur.r[i]; x[a] = q.x; y[a] = q.y; z[a] = q.z; id[a] = (uint32_t)q.w; }   // one 128-bit load, not gated on the species
-    }
-#pragma unroll
-    for (int a = 0; a < kK1Unroll; ++a) {
-      key[a] = 0xFFFFFFFFu;
-      if (s[a] == kDead) continue;
-      const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
-      key[a] = cell_key(m.x, m.y, m.z, p);
-      if (kPack) dsp[a] = pack_disp(m.x - x[a], m.y - y[a], m.z - z[a], m.s != s[a]);
-    }
-    uint32_t first[kK1Unroll], rank[kK1Unroll];
-    int leader[kK1Unroll];
-#pragma unroll
-    for (int a = 0; a < kK1Unroll; ++a) {
-      uint32_t count;
-      run_of_key(key[a], lane, leader[a], rank[a], count);
-      first[a] = 0;
-      if (s[a] != kDead && (int)lane == leader[a]) first[a] = atomicAdd(&p.cell[key[a]], count);
-    }
-#pragma unroll
-    for (int a = 0; a < kK1Unroll; ++a) {
-      const uint32_t f = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]);
-      if (s[a] != kDead) {
-        p.off[base + a * kMoveThreads + threadIdx.x] = f + rank[a];
-        if (kPack) p.disp[base + a * kMoveThreads + threadIdx.x] = dsp[a];
-      }
-    }
-  }
-}
 
 // Test hook (sim_debug_move_only): phase 1 in place on the current arrays.
 template <bool kGaussSmem>
@@ -321,22 +239,28 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(uint32_t* __restrict
 
 // ----------------------------------------------------------------------------- K3 move + scatter / reorder
 // Counting-sort scatter that reorders the whole structure of arrays into cell order (a5), applying
-// phase 1 on the way (move_agent again: same result as in K1, so the same cell), and drops DEAD
-// slots, which is the compaction of the previous step's deaths (fused, a9).  Same tiling as K1:
-// kK3Unroll agents in flight per thread.  Membrane crossings change the species here; their
-// counts deltas go straight to counts row t+1 (rare events).
-template <bool kGaussSmem, int kK3Unroll, int kMinBlk, bool kPack>
+// phase 1 on the way (move_agent again: same result as in the histogram pass, so the same cell), and drops
+// DEAD slots, which is the compaction of the previous step's deaths (fused, a9).  The cell array holds, after
+// the scan, the first slot of every cell one word ahead (cursor[k] = cell[k + 1]); a run of equal keys in a
+// warp takes its slots with one atomicAdd on that cursor, so when the kernel ends cursor[k] is the END of
+// cell k = the start of cell k + 1, i.e. cell[k] = start of cell k and cell[n_cells] = live agents, which is
+// what every later kernel reads.  No per-agent rank array is written or read.  kK3Unroll agents in flight per
+// thread.  Membrane crossings change the species here; their counts deltas go straight to counts row t+1
+// (rare events).
+template <bool kGaussSmem, int kK3Unroll, int kMinBlk>
 __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
   extern __shared__ __align__(16) int16_t s_gauss[];
   __shared__ MoveTables M;
-  const int16_t* g = stage_tables<kGaussSmem && !kPack>(p, M, s_gauss);
+  const int16_t* g = stage_tables<kGaussSmem>(p, M, s_gauss);
   const uint32_t n = p.scal->n_slots, t = p.scal->t;
+  const uint32_t lane = threadIdx.x & 31u;
+  uint32_t* __restrict__ cursor = p.cell + 1;
   uint32_t* __restrict__ row = p.counts + (size_t)(t + 1) * p.row_width;
   constexpr uint32_t kTile = kMoveThreads * kK3Unroll;
-  for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {
+  for (uint32_t base = blockIdx.x * kTile; base < n; base += gridDim.x * kTile) {   // block-uniform trip count
     uint16_t s[kK3Unroll];
     int32_t x[kK3Unroll], y[kK3Unroll], z[kK3Unroll];
-    uint32_t id[kK3Unroll], off[kK3Unroll], dsp[kK3Unroll];
+    uint32_t id[kK3Unroll], key[kK3Unroll];
 #pragma unroll
     for (int a = 0; a < kK3Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
@@ -345,33 +269,34 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
 #pragma unroll
     for (int a = 0; a < kK3Unroll; ++a) {
       const uint32_t i = base + a * kMoveThreads + threadIdx.x;
-      if (i < n) {   // not gated on the species: one round trip
-        const int4 q = p.cur.r[i]; x[a] = q.x; y[a] = q.y; z[a] = q.z; id[a] = (uint32_t)q.w; off[a] = p.off[i];
-        if (kPack) dsp[a] = p.disp[i];
-      }
+      if (i < n) { const int4 q = p.cur.r[i]; x[a] = q.x; y[a] = q.y; z[a] = q.z; id[a] = (uint32_t)q.w; }   // not gated on the species: one round trip
     }
 #pragma unroll
     for (int a = 0; a < kK3Unroll; ++a) {
+      key[a] = 0xFFFFFFFFu;
       if (s[a] == kDead) continue;
-      Moved m;
-      if (kPack) {
-        m.x = x[a] + unpack10(dsp[a], 0); m.y = y[a] + unpack10(dsp[a], 10); m.z = z[a] + unpack10(dsp[a], 20);
-        m.s = (dsp[a] >> 30 & 1u) ? M.sp[s[a]].cross_to : s[a];
-      } else {
-        m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
-      }
+      const Moved m = move_agent(p, M, g, s[a], x[a], y[a], z[a], id[a], t);
       if (m.s != s[a]) {
         const uint32_t rep = (uint32_t)x[a] >> p.stride_shift;
         atomicSub(&row[rep * p.n_species + s[a]], 1u);
         atomicAdd(&row[rep * p.n_species + m.s], 1u);
       }
       x[a] = m.x; y[a] = m.y; z[a] = m.z; s[a] = m.s;
-      off[a] += p.cell[cell_key(m.x, m.y, m.z, p)];
+      key[a] = cell_key(m.x, m.y, m.z, p);
+    }
+    uint32_t first[kK3Unroll], rank[kK3Unroll];
+    int leader[kK3Unroll];
+#pragma unroll
+    for (int a = 0; a < kK3Unroll; ++a) {
+      uint32_t count;
+      run_of_key(key[a], lane, leader[a], rank[a], count);
+      first[a] = 0;
+      if (s[a] != kDead && (int)lane == leader[a]) first[a] = atomicAdd(&cursor[key[a]], count);
     }
 #pragma unroll
     for (int a = 0; a < kK3Unroll; ++a) {
+      const uint32_t dst = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]) + rank[a];
       if (s[a] == kDead) continue;
-      const uint32_t dst = off[a];
       p.oth.r[dst] = make_int4(x[a], y[a], z[a], (int32_t)id[a]);     // ONE scattered 128-bit store per agent
       p.oth.sp[dst] = s[a];
     }
@@ -783,15 +708,24 @@ __global__ void __launch_bounds__(256) k_resolve(const __grid_constant__ Params 
   delta_flush(s_delta, p.counts + (size_t)(t + 1) * p.row_width, p.row_width);
 }
 
-// ----------------------------------------------------------------------------- K5 unimolecular
+// ----------------------------------------------------------------------------- K5 unimolecular + next histogram
 // Phase 3 (a8): per agent, per channel, Philox(seed, t, id) word < threshold.  Most agents belong to
 // a species without channels: a thread reads the species of 8 agents with one 128-bit load; the
 // slots of those that have channels (chan_mask) are compacted into a shared list and only these
 // are processed, one per thread, so the Philox work is dense.  Species are rewritten in place only
-// where they change.  The same pass clears the proposal state K4 left (hasprop byte -> best[]).  Firing parents are appended to the birth list and flagged in the
-// id-indexed birth bitmap (4 bits per id) that K6 ranks.  Counts deltas are block-aggregated.
+// where they change.  The same pass clears the proposal state K4 left (hasprop byte -> best[]).  Firing parents
+// are appended to the birth list and flagged in the id-indexed birth bitmap (4 bits per id) that K6 ranks.
+// Counts deltas are block-aggregated.
+//
+// With the species of the tile final (nothing after this pass changes a sorted agent), the same kernel takes the
+// cell histogram of step t+1 (a3): move_agent() for step t+1 gives the cell every survivor will be sorted into,
+// and a run of equal keys in a warp adds its length to that cell's counter (fire-and-forget atomics into the
+// OTHER cell array, zeroed meanwhile).  The next step therefore starts at its scan: the separate histogram
+// pass of round 1, its rank array and one launch are gone, and the species are streamed once for both jobs.
+// Newborns are counted by K6, which places them.  With kUni = false the kernel is only the histogram pass, of
+// the CURRENT arrays for the current step: the prologue after seeding / loading.
 __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __restrict__ T, uint32_t i, uint16_t s0,
-                                        uint32_t t, int32_t* s_delta) {
+                                        uint32_t t, int32_t* s_delta, uint16_t* s_sp_slot) {
   const DevSpecies& S = T->sp[s0];
   const uint32_t nch = S.n_channels;
   const uint32_t id = (uint32_t)p.oth.r[i].w;
@@ -828,6 +762,7 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
   int32_t* d = s_delta + ((uint32_t)p.oth.r[i].x >> p.stride_shift) * p.n_species;
   if (s != s0) {
     p.oth.sp[i] = s;
+    *s_sp_slot = s;                        // the tile copy the histogram part reads
     atomicSub(&d[s0], 1);
     if (s != kDead) atomicAdd(&d[s], 1);
   }
@@ -843,169 +778,208 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
 
 constexpr int kUniThreads = 256;
 constexpr int kUniTile = kUniThreads * 8;
-__global__ void __launch_bounds__(kUniThreads) k_uni(Params p) {
-  __shared__ int32_t s_delta[kMaxRowWidth];
-  __shared__ uint16_t s_list[kUniTile];      // tile-local slots of the agents that have channels
+// Dynamic shared memory: [Gaussian tables (if kGaussSmem)] [counts deltas, row_width words (if kUni)].
+template <bool kGaussSmem, bool kUni, int kMinBlk>
+__global__ void __launch_bounds__(kUniThreads, kMinBlk) k_uni_hist(Params p) {
+  extern __shared__ __align__(16) int16_t s_dyn[];
+  __shared__ MoveTables M;
+  __shared__ __align__(16) uint16_t s_sp[kUniTile];   // species of the tile, after the unimolecular reactions
+  __shared__ uint16_t s_list[kUni ? kUniTile : 1];     // tile-local slots of the agents that have channels
   __shared__ uint32_t s_n;
-  delta_zero(s_delta, p.row_width);
-  const uint32_t n = p.cell[p.n_cells], t = p.scal->t;
+  const int16_t* g = stage_tables<kGaussSmem>(p, M, s_dyn);
+  int32_t* s_delta = reinterpret_cast<int32_t*>(s_dyn + (kGaussSmem ? (((p.n_classes << p.table_bits) + 7u) & ~7u) : 0u));
+  if (kUni) delta_zero(s_delta, p.row_width);
+  const Soa src = kUni ? p.oth : p.cur;
+  uint32_t* __restrict__ hist = (kUni ? p.cell_next : p.cell) + 1;
+  const uint32_t n = kUni ? p.cell[p.n_cells] : p.scal->n_slots;
+  const uint32_t t = p.scal->t, t_move = kUni ? t + 1u : t;
   const DevTables* __restrict__ T = p.tab;
   const uint32_t lane = threadIdx.x & 31u;
   for (uint32_t base = blockIdx.x * kUniTile; base < n; base += gridDim.x * kUniTile) {   // block-uniform
-    if (threadIdx.x == 0) s_n = 0;
-    __syncthreads();
-    const uint32_t l0 = threadIdx.x * 8u, i0 = base + l0;
-    uint32_t w[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
-    if (i0 + 8u <= n) {
-      const uint4 q = *reinterpret_cast<const uint4*>(p.oth.sp + i0);
-      w[0] = q.x; w[1] = q.y; w[2] = q.z; w[3] = q.w;
-    } else {
-      for (uint32_t k = 0; i0 + k < n; ++k) {
-        const uint32_t v = p.oth.sp[i0 + k];
-        w[k >> 1] = (k & 1u) ? ((w[k >> 1] & 0x0000FFFFu) | (v << 16)) : ((w[k >> 1] & 0xFFFF0000u) | v);
+    if (kUni) {
+      if (threadIdx.x == 0) s_n = 0;
+      __syncthreads();                      // also: the previous tile's readers of s_sp / s_list are done
+      const uint32_t l0 = threadIdx.x * 8u, i0 = base + l0;
+      uint32_t w[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+      if (i0 + 8u <= n) {
+        const uint4 q = *reinterpret_cast<const uint4*>(src.sp + i0);
+        w[0] = q.x; w[1] = q.y; w[2] = q.z; w[3] = q.w;
+      } else {
+        for (uint32_t k = 0; i0 + k < n; ++k) {
+          const uint32_t v = src.sp[i0 + k];
+          w[k >> 1] = (k & 1u) ? ((w[k >> 1] & 0x0000FFFFu) | (v << 16)) : ((w[k >> 1] & 0xFFFF0000u) | v);
+        }
+      }
+      *reinterpret_cast<uint4*>(s_sp + l0) = make_uint4(w[0], w[1], w[2], w[3]);
+      // this step's proposals are resolved: put the touched best[] entries back to "none" for the next K4
+      if (i0 < n) {
+        uint8_t* hp = reinterpret_cast<uint8_t*>(p.hasprop) + (i0 >> 3);
+        uint32_t bits = *hp;
+        if (bits) {
+          *hp = 0;
+          while (bits) { p.best[i0 + __ffs(bits) - 1u] = kNoKey; bits &= bits - 1u; }
+        }
+      }
+      uint32_t mask = 0;
+#pragma unroll
+      for (uint32_t k = 0; k < 8u; ++k) {
+        const uint32_t s = (w[k >> 1] >> ((k & 1u) * 16u)) & 0xFFFFu;
+        if (s != kDead && ((p.chan_mask >> s) & 1ull)) mask |= 1u << k;
+      }
+      // compact: warp-inclusive scan of the counts, one shared atomic per warp
+      const uint32_t cnt = __popc(mask);
+      uint32_t incl = cnt;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+        if (lane >= (uint32_t)d) incl += o;
+      }
+      const uint32_t wtotal = __shfl_sync(0xFFFFFFFFu, incl, 31);
+      uint32_t wbase = 0;
+      if (lane == 31 && wtotal) wbase = atomicAdd(&s_n, wtotal);
+      wbase = __shfl_sync(0xFFFFFFFFu, wbase, 31);
+      uint32_t pos = wbase + incl - cnt;
+      while (mask) {
+        s_list[pos++] = (uint16_t)(l0 + __ffs(mask) - 1u);
+        mask &= mask - 1u;
+      }
+      __syncthreads();
+      const uint32_t m = s_n;
+      for (uint32_t k = threadIdx.x; k < m; k += kUniThreads) {
+        const uint32_t l = s_list[k];
+        uni_one(p, T, base + l, s_sp[l], t, s_delta, &s_sp[l]);
+      }
+      __syncthreads();                      // the tile's species are final
+    }
+    // ---- cell histogram of the step that moves these agents next: two batches of four agents in flight
+#pragma unroll
+    for (uint32_t half = 0; half < 2u; ++half) {
+      uint16_t s[4];
+      int4 q[4];
+      uint32_t key[4];
+#pragma unroll
+      for (uint32_t a = 0; a < 4u; ++a) {
+        const uint32_t l = (half * 4u + a) * kUniThreads + threadIdx.x, i = base + l;
+        s[a] = kDead;
+        if (i < n) { s[a] = kUni ? s_sp[l] : src.sp[i]; q[a] = src.r[i]; }   // the record load is not gated on the species
+      }
+#pragma unroll
+      for (uint32_t a = 0; a < 4u; ++a) {
+        key[a] = 0xFFFFFFFFu;
+        if (s[a] == kDead) continue;
+        const Moved m = move_agent(p, M, g, s[a], q[a].x, q[a].y, q[a].z, (uint32_t)q[a].w, t_move);
+        key[a] = cell_key(m.x, m.y, m.z, p);
+      }
+#pragma unroll
+      for (uint32_t a = 0; a < 4u; ++a) {
+        int leader; uint32_t rank, count;
+        run_of_key(key[a], lane, leader, rank, count);
+        if (s[a] != kDead && rank == 0u) atomicAdd(&hist[key[a]], count);     // result unused: a reduction, no round trip
       }
     }
-    // this step's proposals are resolved: put the touched best[] entries back to "none" for the next K4
-    if (i0 < n) {
-      uint8_t* hp = reinterpret_cast<uint8_t*>(p.hasprop) + (i0 >> 3);
-      uint32_t bits = *hp;
-      if (bits) {
-        *hp = 0;
-        while (bits) { p.best[i0 + __ffs(bits) - 1u] = kNoKey; bits &= bits - 1u; }
-      }
-    }
-    uint32_t mask = 0;
-#pragma unroll
-    for (uint32_t k = 0; k < 8u; ++k) {
-      const uint32_t s = (w[k >> 1] >> ((k & 1u) * 16u)) & 0xFFFFu;
-      if (s != kDead && ((p.chan_mask >> s) & 1ull)) mask |= 1u << k;
-    }
-    // compact: warp-inclusive scan of the counts, one shared atomic per warp
-    const uint32_t cnt = __popc(mask);
-    uint32_t incl = cnt;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-      if (lane >= (uint32_t)d) incl += o;
-    }
-    const uint32_t wtotal = __shfl_sync(0xFFFFFFFFu, incl, 31);
-    uint32_t wbase = 0;
-    if (lane == 31 && wtotal) wbase = atomicAdd(&s_n, wtotal);
-    wbase = __shfl_sync(0xFFFFFFFFu, wbase, 31);
-    uint32_t pos = wbase + incl - cnt;
-    while (mask) {
-      s_list[pos++] = (uint16_t)(l0 + __ffs(mask) - 1u);
-      mask &= mask - 1u;
-    }
-    __syncthreads();
-    const uint32_t m = s_n;
-    for (uint32_t k = threadIdx.x; k < m; k += kUniThreads) {
-      const uint32_t i = base + s_list[k];
-      uni_one(p, T, i, p.oth.sp[i], t, s_delta);
-    }
-    __syncthreads();   // s_list / s_n are reused by the next tile
   }
-  delta_flush(s_delta, p.counts + (size_t)(t + 1) * p.row_width, p.row_width);
+  if (kUni) delta_flush(s_delta, p.counts + (size_t)(t + 1) * p.row_width, p.row_width);
 }
 
-// ----------------------------------------------------------------------------- K6 births
+// ----------------------------------------------------------------------------- K6 births + epilogue
 // New ids are assigned in (parent id, channel) order (north_star (5), S14).  The birth bitmap (4 bits
 // per id) is indexed by parent id, so a newborn's rank is the number of set bits below its own; K5
 // also keeps the newborn count of every block of 256 ids (birth_mid) and of every 2^top_shift ids
 // (birth_top, at most kMaxTop entries).  One launch: every block scans birth_top into shared memory,
 // then one warp per firing parent adds the birth_mid entries and bitmap words between the block
 // boundaries and the parent (a few dozen coalesced loads per lane at most) and lanes 0..3 place the
-// newborns (phase 4, a9): newborn g of the step gets id next_id + g and slot n_sorted + g.
+// newborns (phase 4, a9): newborn g of the step gets id next_id + g and slot n_sorted + g, and is counted in the
+// next step's cell histogram like every survivor (K5).  The last block to finish then clears the touched
+// birth-bitmap words and counters, advances the device scalars and seeds counts row t+2 with row t+1 (the
+// next step adds its deltas to it; a10).
 __global__ void __launch_bounds__(kScanThreads) k_births(Params p) {
   __shared__ uint32_t s_warp[9];
   __shared__ uint32_t s_top[kMaxTop];
-  const uint32_t nb = p.scal->birth_count;
-  if (nb == 0) {
-    if (blockIdx.x == 0 && threadIdx.x == 0) p.scal->total_births = 0;
-    return;
-  }
-  const uint32_t next_id = p.scal->next_id, t = p.scal->t;
-  const uint32_t n_top = ((next_id - 1u) >> p.top_shift) + 1u;          // parents have ids < next_id
-  constexpr uint32_t kPer = kMaxTop / kScanThreads;
-  uint32_t v[kPer], sum = 0;
-#pragma unroll
-  for (uint32_t k = 0; k < kPer; ++k) {
-    const uint32_t j = threadIdx.x * kPer + k;
-    v[k] = j < n_top ? p.birth_top[j] : 0u;
-    sum += v[k];
-  }
-  uint32_t total;
-  uint32_t e0 = block_excl_scan(sum, total, s_warp);
-#pragma unroll
-  for (uint32_t k = 0; k < kPer; ++k) { s_top[threadIdx.x * kPer + k] = e0; e0 += v[k]; }
-  __syncthreads();
-  const uint32_t n_sorted = p.cell[p.n_cells];
-  uint32_t bad = 0;
-  if ((unsigned long long)n_sorted + total > p.capacity) bad |= 1u;
-  if ((unsigned long long)next_id + total > p.id_capacity) bad |= 2u;
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    p.scal->total_births = total;
-    if (bad) atomicOr(&p.scal->err, bad);
-  }
-  if (bad) return;
-  const DevTables* __restrict__ T = p.tab;
-  const uint32_t lane = threadIdx.x & 31u, wpb = kScanThreads / 32;
-  for (uint32_t e = blockIdx.x * wpb + (threadIdx.x >> 5); e < nb; e += gridDim.x * wpb) {
-    const uint2 ent = p.birth_list[e];
-    const uint32_t slot = ent.x, mask = ent.y & 0xFu, pre = ent.y >> 16;
-    const uint32_t pid = (uint32_t)p.oth.r[slot].w;
-    uint32_t part = 0;
-    for (uint32_t j = ((pid >> p.top_shift) << (p.top_shift - kMidShift)) + lane; j < (pid >> kMidShift); j += 32u)
-      part += p.birth_mid[j];
-    const uint32_t w0 = (pid >> kMidShift) << (kMidShift - 3u), w1 = pid >> 3;      // bitmap words of this 256-id block
-    if (w0 + lane < w1) part += __popc(p.bits[w0 + lane]);
-    if (lane == 31u) part += __popc(p.bits[w1] & ((1u << ((pid & 7u) * 4u)) - 1u));
-    const uint32_t rank0 = s_top[pid >> p.top_shift] + __reduce_add_sync(0xFFFFFFFFu, part);
-    if (lane < 4u && (mask >> lane & 1u)) {
-      const uint32_t k = lane, rank = rank0 + __popc(mask & ((1u << k) - 1u));
-      const int4 qp = p.oth.r[slot];
-      const int32_t px = qp.x, py = qp.y, pz = qp.z;
-      const int32_t rbase = (int32_t)(((uint32_t)px >> p.stride_shift) << p.stride_shift);
-      const int32_t lx = px - rbase;
-      const uint16_t sp_new = T->sp[pre].ch[k].prod1;
-      const uint4 r = philox_sim(p, pid, k, t, kTagBirth);
-      int32_t qx = lx + (int32_t)__umulhi(r.x, 21u) - 10;
-      int32_t qy = py + (int32_t)__umulhi(r.y, 21u) - 10;
-      int32_t qz = pz + (int32_t)__umulhi(r.z, 21u) - 10;
-      const DevComp& c = T->comp[T->sp[sp_new].compartment];
-      if (c.shape == 0) { qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L); }
-      else if (!comp_valid(c, qx, qy, qz)) { qx = lx; qy = py; qz = pz; }
-      const uint32_t dst = n_sorted + rank;
-      p.oth.r[dst] = make_int4(qx + rbase, qy, qz, (int32_t)(next_id + rank));
-      p.oth.sp[dst] = sp_new;
-    }
-  }
-}
-
-// ----------------------------------------------------------------------------- K7 epilogue
-// Clears the touched birth-bitmap words and counters; the last block to finish advances the device scalars and
-// seeds counts row t+2 with row t+1 (the next step adds its deltas to it; a10).
-__global__ void __launch_bounds__(256) k_epilogue(Params p) {
+  __shared__ MoveTables M;
   __shared__ uint32_t s_last;
   const uint32_t nb = p.scal->birth_count;
-  const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < nb; e += stride) {
-    const uint32_t pid = (uint32_t)p.oth.r[p.birth_list[e].x].w;
-    p.bits[pid >> 3] = 0u; p.birth_mid[pid >> kMidShift] = 0u; p.birth_top[pid >> p.top_shift] = 0u;
+  const uint32_t n_sorted = p.cell[p.n_cells];
+  const uint32_t t = p.scal->t;
+  uint32_t total = 0;
+  bool bad_any = false;
+  if (nb) {             // block-uniform
+    stage_tables<false>(p, M, nullptr);
+    const uint32_t next_id = p.scal->next_id;
+    const uint32_t n_top = ((next_id - 1u) >> p.top_shift) + 1u;          // parents have ids < next_id
+    constexpr uint32_t kPer = kMaxTop / kScanThreads;
+    uint32_t v[kPer], sum = 0;
+#pragma unroll
+    for (uint32_t k = 0; k < kPer; ++k) {
+      const uint32_t j = threadIdx.x * kPer + k;
+      v[k] = j < n_top ? p.birth_top[j] : 0u;
+      sum += v[k];
+    }
+    uint32_t e0 = block_excl_scan(sum, total, s_warp);
+#pragma unroll
+    for (uint32_t k = 0; k < kPer; ++k) { s_top[threadIdx.x * kPer + k] = e0; e0 += v[k]; }
+    __syncthreads();
+    uint32_t bad = 0;
+    if ((unsigned long long)n_sorted + total > p.capacity) bad |= 1u;
+    if ((unsigned long long)next_id + total > p.id_capacity) bad |= 2u;
+    if (bad && blockIdx.x == 0 && threadIdx.x == 0) atomicOr(&p.scal->err, bad);
+    bad_any = bad != 0u;
+    if (!bad) {
+      const DevTables* __restrict__ T = p.tab;
+      uint32_t* __restrict__ hist = p.cell_next + 1;
+      const uint32_t lane = threadIdx.x & 31u, wpb = kScanThreads / 32;
+      for (uint32_t e = blockIdx.x * wpb + (threadIdx.x >> 5); e < nb; e += gridDim.x * wpb) {
+        const uint2 ent = p.birth_list[e];
+        const uint32_t slot = ent.x, mask = ent.y & 0xFu, pre = ent.y >> 16;
+        const uint32_t pid = (uint32_t)p.oth.r[slot].w;
+        uint32_t part = 0;
+        for (uint32_t j = ((pid >> p.top_shift) << (p.top_shift - kMidShift)) + lane; j < (pid >> kMidShift); j += 32u)
+          part += p.birth_mid[j];
+        const uint32_t w0 = (pid >> kMidShift) << (kMidShift - 3u), w1 = pid >> 3;      // bitmap words of this 256-id block
+        if (w0 + lane < w1) part += __popc(p.bits[w0 + lane]);
+        if (lane == 31u) part += __popc(p.bits[w1] & ((1u << ((pid & 7u) * 4u)) - 1u));
+        const uint32_t rank0 = s_top[pid >> p.top_shift] + __reduce_add_sync(0xFFFFFFFFu, part);
+        if (lane < 4u && (mask >> lane & 1u)) {
+          const uint32_t k = lane, rank = rank0 + __popc(mask & ((1u << k) - 1u));
+          const int4 qp = p.oth.r[slot];
+          const int32_t px = qp.x, py = qp.y, pz = qp.z;
+          const int32_t rbase = (int32_t)(((uint32_t)px >> p.stride_shift) << p.stride_shift);
+          const int32_t lx = px - rbase;
+          const uint16_t sp_new = T->sp[pre].ch[k].prod1;
+          const uint4 r = philox_sim(p, pid, k, t, kTagBirth);
+          int32_t qx = lx + (int32_t)__umulhi(r.x, 21u) - 10;
+          int32_t qy = py + (int32_t)__umulhi(r.y, 21u) - 10;
+          int32_t qz = pz + (int32_t)__umulhi(r.z, 21u) - 10;
+          const DevComp& c = T->comp[T->sp[sp_new].compartment];
+          if (c.shape == 0) { qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L); }
+          else if (!comp_valid(c, qx, qy, qz)) { qx = lx; qy = py; qz = pz; }
+          const uint32_t dst = n_sorted + rank;
+          p.oth.r[dst] = make_int4(qx + rbase, qy, qz, (int32_t)(next_id + rank));
+          p.oth.sp[dst] = sp_new;
+          // the newborn's cell in the next step's sort
+          const Moved m = move_agent(p, M, p.gauss, sp_new, qx + rbase, qy, qz, next_id + rank, t + 1u);
+          atomicAdd(&hist[cell_key(m.x, m.y, m.z, p)], 1u);
+        }
+      }
+    }
   }
+  // ---- epilogue, by the last block to get here (every block's births are placed and its bitmap reads are done)
   __threadfence();
   __syncthreads();
   if (threadIdx.x == 0) s_last = atomicAdd(&p.scal->ticket, 1u) == gridDim.x - 1 ? 1u : 0u;
   __syncthreads();
   if (!s_last) return;
+  __threadfence();
+  for (uint32_t e = threadIdx.x; e < nb; e += blockDim.x) {
+    const uint32_t pid = (uint32_t)p.oth.r[p.birth_list[e].x].w;
+    p.bits[pid >> 3] = 0u; p.birth_mid[pid >> kMidShift] = 0u; p.birth_top[pid >> p.top_shift] = 0u;
+  }
   Scalars* sc = p.scal;
-  const uint32_t t = sc->t;
   const uint32_t* src = p.counts + (size_t)(t + 1) * p.row_width;
   uint32_t* dst = p.counts + (size_t)(t + 2) * p.row_width;
   for (uint32_t k = threadIdx.x; k < p.row_width; k += blockDim.x) dst[k] = __ldcg(src + k);
   if (threadIdx.x == 0) {
-    const uint32_t add = sc->err ? 0u : sc->total_births;
-    sc->n_slots = p.cell[p.n_cells] + add;
+    const uint32_t add = (bad_any || sc->err) ? 0u : total;
+    sc->n_slots = n_sorted + add;
     sc->next_id += add;
     sc->t = t + 1;
     sc->birth_count = 0; sc->total_births = 0; sc->ticket = 0;

@@ -19,16 +19,16 @@ namespace {
 constexpr uint32_t kMaxScanBlocks = 592;  // 148 SMs x 4; small problems get proportionally smaller grids (launch-bound)
 constexpr uint32_t kMaxTailBlocks = 148;
 
-enum KernelId { KI_MOVE = 0, KI_CELL_ZERO, KI_CELL_REDUCE, KI_CELL_SCAN, KI_SCATTER, KI_PAIRS,
-                KI_RESOLVE, KI_UNI, KI_BIRTHS, KI_EPILOGUE, KI_OTHER };
+enum KernelId { KI_HIST = 0, KI_CELL_ZERO, KI_CELL_REDUCE, KI_CELL_SCAN, KI_SCATTER, KI_PAIRS,
+                KI_RESOLVE, KI_UNI_HIST, KI_BIRTHS, KI_OTHER };
 const char* kKernelNames[SIM_N_KERNELS] = {
-    "k_move_hist", "memset_cells", "k_cell_reduce", "k_cell_scan", "k_scatter", "k_pairs",
-    "k_resolve", "k_uni", "k_births", "k_epilogue", "other"};
+    "k_hist_prologue", "memset_cells", "k_cell_reduce", "k_cell_scan", "k_scatter", "k_pairs",
+    "k_resolve", "k_uni_hist", "k_births", "other"};
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t soa[2][2], off, disp, prop, best, hasprop, cell, partial, bits, birth_mid, birth_top, birth_list, counts,
+  size_t soa[2][2], prop, best, hasprop, cell[2], partial, bits, birth_mid, birth_top, birth_list, counts,
       scal, tab, gauss, total;
   uint32_t n_cells, nx, ny, nz;
 };
@@ -44,10 +44,12 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   const size_t cap = c->capacity;
   // records, species; the slack covers the tile (+ halo) that K4's bulk copies read past the last slot
   for (int b = 0; b < 2; ++b) { L.soa[b][0] = take(cap * 16 + (kPairThreads + kPairHalo) * 16); L.soa[b][1] = take(cap * 2 + kPairThreads * 2); }
-  L.off = take(cap * 4); L.disp = take(cap * 4); L.prop = take(cap * 4);
+  L.prop = take(cap * 4);
   L.best = take(cap * 8);
   L.hasprop = take((cap / 32 + 16) * 4);
-  L.cell = take(((size_t)nc + 1 + 1024) * 4);
+  // two cell arrays (this step's and the next step's histogram); 4 words of lead so that the counts, which start one
+  // word behind the leading zero, are 16-byte aligned; slack for the look-ups K4 makes past the last row
+  for (int b = 0; b < 2; ++b) L.cell[b] = take(((size_t)nc + 8 + 1024) * 4);
   L.partial = take(4096 * 4);
   const size_t n_chunks = ((size_t)c->id_capacity + 63) / 64 + 1;
   L.bits = take(n_chunks * 8 * 4);
@@ -148,12 +150,15 @@ struct sim {
   uint32_t t_host = 0;           // steps enqueued so far (the host knows t exactly)
   uint64_t launches = 0;
   int gauss_in_smem = 0;
-  void (*k_move)(Params) = nullptr;   // K1 / K3 instantiation picked at create time (Gaussian tables in shared
-  void (*k_scat)(Params) = nullptr;   // memory or not; MoveCfgSmall or MoveCfgLarge)
-  uint32_t k1_unroll = 0, k3_unroll = 0;
-  bool pack_disp = false;             // every table entry fits 10 signed bits: K1 hands the displacement to K3
-  size_t gauss_bytes = 0;
-  uint32_t grid_move = 0, grid_scatter = 0, grid_pairs = 0, grid_uni = 0, grid_resolve = 0;
+  void (*k_scat)(Params) = nullptr;   // K3 / K5 / prologue instantiations picked at create time (Gaussian tables in
+  void (*k_unih)(Params) = nullptr;   // shared memory or not; small- or large-population launch shape)
+  void (*k_hist)(Params) = nullptr;
+  uint32_t k3_unroll = 0;
+  size_t gauss_bytes = 0, unih_smem = 0;
+  uint32_t grid_scatter = 0, grid_pairs = 0, grid_unih = 0, grid_resolve = 0;
+  bool hist_valid = false;            // prm.cell holds the histogram of the current state for the current step
+  cudaStream_t side = nullptr;        // zeroes the next cell array beside K3 / K4 (a parallel branch of the step graph)
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   uint32_t cell_seg = 0, scan_blocks = 1, tail_blocks = 1;
   bool profile = false;
   float prof_ms[SIM_N_KERNELS] = {};
@@ -219,26 +224,38 @@ int recount_row(sim* s, uint32_t r, uint32_t n_slots) {
   return SIM_OK;
 }
 
+// Histogram of the CURRENT arrays for the current step (after seeding / loading; a step leaves the next one's behind).
+int enqueue_prologue(sim* s) {
+  Params& p = s->prm;
+  CK(cudaMemsetAsync(p.cell - 3, 0, ((size_t)p.n_cells + 8) * 4, s->stream));
+  { ProfScope ps(s, KI_HIST);
+    s->k_hist<<<s->grid_unih, kUniThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->stream>>>(p); }
+  CK(cudaGetLastError());
+  s->hist_valid = true;
+  return SIM_OK;
+}
+
 int enqueue_step(sim* s) {
   Params& p = s->prm;
-  {
-    ProfScope ps(s, KI_CELL_ZERO, false);
-    CK(cudaMemsetAsync(p.cell, 0, ((size_t)p.n_cells + 1) * 4, s->run));
-  }
-  { ProfScope ps(s, KI_MOVE); s->k_move<<<s->grid_move, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p); }
+  // the next step's cell array is zeroed on the side stream while K2 .. K4b run (its last readers were the previous step's)
+  CK(cudaEventRecord(s->ev_fork, s->run));
+  CK(cudaStreamWaitEvent(s->side, s->ev_fork, 0));
+  CK(cudaMemsetAsync(p.cell_next - 3, 0, ((size_t)p.n_cells + 8) * 4, s->side));
+  CK(cudaEventRecord(s->ev_join, s->side));
   { ProfScope ps(s, KI_CELL_REDUCE);
-    k_cell_reduce<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+    k_cell_reduce<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell + 1, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_CELL_SCAN);
-    k_cell_scan<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell, p.n_cells, s->cell_seg, p.partial); }
+    k_cell_scan<<<s->scan_blocks, kScanThreads, 0, s->run>>>(p.cell + 1, p.n_cells, s->cell_seg, p.partial); }
   { ProfScope ps(s, KI_SCATTER);
-    s->k_scat<<<s->grid_scatter, kMoveThreads, (s->gauss_in_smem && !s->pack_disp) ? s->gauss_bytes : 0, s->run>>>(p); }
+    s->k_scat<<<s->grid_scatter, kMoveThreads, s->gauss_in_smem ? s->gauss_bytes : 0, s->run>>>(p); }
   { ProfScope ps(s, KI_PAIRS); k_pairs<<<s->grid_pairs, kPairBlock, 0, s->run>>>(p); }
   { ProfScope ps(s, KI_RESOLVE); k_resolve<<<s->grid_resolve, 256, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_UNI); k_uni<<<s->grid_uni, 256, 0, s->run>>>(p); }
+  CK(cudaStreamWaitEvent(s->run, s->ev_join, 0));
+  { ProfScope ps(s, KI_UNI_HIST); s->k_unih<<<s->grid_unih, kUniThreads, s->unih_smem, s->run>>>(p); }
   { ProfScope ps(s, KI_BIRTHS); k_births<<<s->tail_blocks, kScanThreads, 0, s->run>>>(p); }
-  { ProfScope ps(s, KI_EPILOGUE); k_epilogue<<<s->tail_blocks, 256, 0, s->run>>>(p); }
   CK(cudaGetLastError());
-  std::swap(p.cur, p.oth);   // the sorted copy (+ newborns) is the next step's current state
+  std::swap(p.cur, p.oth);   // the sorted copy (+ newborns) is the next step's current state,
+  std::swap(p.cell, p.cell_next);   // and its histogram has been taken
   s->t_host++;
   return SIM_OK;
 }
@@ -249,6 +266,7 @@ namespace {
 
 constexpr uint32_t kGraphSteps = 8;   // even, so the parity after the graph equals the parity before
 
+void flip(sim* s) { std::swap(s->prm.cur, s->prm.oth); std::swap(s->prm.cell, s->prm.cell_next); }
 int parity_of(const sim* s) { return s->prm.cur.r == (const int4*)(s->ws + s->lay.soa[0][0]) ? 0 : 1; }
 
 // Captures `steps` steps starting at the current parity into an executable graph; the handle's
@@ -273,7 +291,7 @@ bool capture_steps(sim* s, uint32_t steps, cudaGraphExec_t* out) {
   return ok;
 }
 
-// The 10 launches of a step are replayed as CUDA graphs (one step, or 8 steps, per starting parity of
+// The 7 launches (+ the memset branch) of a step are replayed as CUDA graphs (one step, or 8 steps, per starting parity of
 // the cur/oth ping-pong): the path is launch-bound below ~1 M agents.
 void build_graphs(sim* s) {
   s->graphs_tried = true;
@@ -282,7 +300,7 @@ void build_graphs(sim* s) {
   for (int k = 0; k < 2 && ok; ++k) {
     const int par = parity_of(s);
     ok = capture_steps(s, 1, &s->g1[par]) && capture_steps(s, kGraphSteps, &s->g8[par]);
-    std::swap(s->prm.cur, s->prm.oth);   // the other parity (swapped back by the second round)
+    flip(s);   // the other parity (flipped back by the second round)
   }
   s->graphs_ok = ok;
 }
@@ -290,10 +308,13 @@ void build_graphs(sim* s) {
 }  // namespace
 
 namespace {
-template <bool kGauss, bool kPack> void pick_move_kernels(sim* s, bool large) {
-  using S_ = MoveCfgSmall; using L_ = MoveCfgLarge;
-  s->k_move = large ? k_move_hist<kGauss, L_::k1u, L_::k1b, kPack> : k_move_hist<kGauss, S_::k1u, S_::k1b, kPack>;
-  s->k_scat = large ? k_scatter<kGauss, L_::k3u, L_::k3b, kPack> : k_scatter<kGauss, S_::k3u, S_::k3b, kPack>;
+// Launch shapes of the two passes that evaluate the move: agents in flight per thread x resident blocks per SM
+// (K3), resident blocks per SM (K5 / prologue); small populations like many thin blocks.
+template <bool kGauss> void pick_move_kernels(sim* s, bool large) {
+  s->k_scat = k_scatter<kGauss, 2, 5>; (void)large;
+  s->k3_unroll = 2;
+  s->k_unih = k_uni_hist<kGauss, true, 5>;
+  s->k_hist = k_uni_hist<kGauss, false, 5>;
 }
 }  // namespace
 
@@ -323,6 +344,9 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   s->ws = (char*)d_workspace;
   s->stream = (cudaStream_t)cuda_stream;
   s->run = s->stream;
+  if (cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming) != cudaSuccess) { sim_destroy(s); return SIM_E_CUDA; }
 
   // host image of the device tables
   std::vector<DevTables> tabv(1);
@@ -363,9 +387,10 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   char* w = s->ws;
   auto soa = [&](int b) { return Soa{(int4*)(w + L.soa[b][0]), (uint16_t*)(w + L.soa[b][1])}; };
   p.cur = soa(0); p.oth = soa(1);
-  p.off = (uint32_t*)(w + L.off); p.disp = (uint32_t*)(w + L.disp); p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
+  p.prop = (uint32_t*)(w + L.prop); p.hasprop = (uint32_t*)(w + L.hasprop);
   p.best = (unsigned long long*)(w + L.best);
-  p.cell = (uint32_t*)(w + L.cell); p.partial = (uint32_t*)(w + L.partial);
+  p.cell = (uint32_t*)(w + L.cell[0]) + 3; p.cell_next = (uint32_t*)(w + L.cell[1]) + 3;   // cell[1] is 16-byte aligned
+  p.partial = (uint32_t*)(w + L.partial);
   p.bits = (uint32_t*)(w + L.bits); p.birth_mid = (uint32_t*)(w + L.birth_mid); p.birth_top = (uint32_t*)(w + L.birth_top);
   p.birth_list = (uint2*)(w + L.birth_list); p.counts = (uint32_t*)(w + L.counts);
   p.scal = (Scalars*)(w + L.scal); p.tab = (const DevTables*)(w + L.tab); p.gauss = (const int16_t*)(w + L.gauss);
@@ -408,14 +433,6 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
 
   s->gauss_bytes = ((size_t)cfg->n_sigma_classes << cfg->table_bits) * 2;
   s->gauss_in_smem = s->gauss_bytes <= 160 * 1024;
-  {
-    int32_t max_tab = 0;
-    for (size_t i = 0; i < ((size_t)cfg->n_sigma_classes << cfg->table_bits); ++i)
-      max_tab = std::max<int32_t>(max_tab, std::abs((int32_t)cfg->tables[i]));
-    // measured: the extra 4 B/agent stream pays while the state is L2-resident (W3 -6 %, W4 1M -3.5 %) and
-    // costs 10 % at 16 M agents, where K1/K3 are sensitive to every additional HBM stream
-    s->pack_disp = max_tab <= 511 && cfg->capacity < kLargeFrom;
-  }
   // persistent grids: resident blocks per SM (occupancy API) x SM count, capped by the work there is
   {
     int dev = 0, sms = 148;
@@ -427,24 +444,21 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
     };
     int occ = 0;
     const size_t gsm = s->gauss_in_smem ? s->gauss_bytes : 0;
-    using S_ = MoveCfgSmall; using L_ = MoveCfgLarge;
     const bool large = cfg->capacity >= kLargeFrom;
-    if (gsm) { if (s->pack_disp) pick_move_kernels<true, true>(s, large); else pick_move_kernels<true, false>(s, large); }
-    else { if (s->pack_disp) pick_move_kernels<false, true>(s, large); else pick_move_kernels<false, false>(s, large); }
-    s->k1_unroll = large ? L_::k1u : S_::k1u; s->k3_unroll = large ? L_::k3u : S_::k3u;
-    if (gsm > 48 * 1024) {
-      cudaFuncSetAttribute(s->k_move, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+    if (gsm) pick_move_kernels<true>(s, large); else pick_move_kernels<false>(s, large);
+    s->unih_smem = align_up(gsm, 16) + (size_t)p.row_width * 4;      // K5: Gaussian tables, then the counts deltas
+    if (s->unih_smem > 48 * 1024) {
       cudaFuncSetAttribute(s->k_scat, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(s->k_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
+      cudaFuncSetAttribute(s->k_unih, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->unih_smem);
       cudaFuncSetAttribute(k_move_only<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm);
     }
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_move, kMoveThreads, gsm);
-    s->grid_move = sized(occ, (uint64_t)kMoveThreads * s->k1_unroll);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_scat, kMoveThreads, s->pack_disp ? 0 : gsm);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_scat, kMoveThreads, gsm);
     s->grid_scatter = sized(occ, (uint64_t)kMoveThreads * s->k3_unroll);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, s->k_unih, kUniThreads, s->unih_smem);
+    s->grid_unih = sized(occ, kUniTile);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pairs, kPairBlock, 0);
     s->grid_pairs = sized(occ, kPairThreads);                  // persistent: tiles are dealt round-robin
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_uni, kUniThreads, 0);
-    s->grid_uni = sized(occ, kUniTile);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_resolve, 256, 0);
     s->grid_resolve = sized(occ, 256 * 32);
     if (cudaGetLastError() != cudaSuccess) { delete s; return SIM_E_CUDA; }
@@ -460,7 +474,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
   bool ok = true;
   ok = ok && cudaMemsetAsync(p.bits, 0, L.birth_list - L.bits, s->stream) == cudaSuccess;
   ok = ok && cudaMemsetAsync(p.best, 0xFF, L.hasprop - L.best, s->stream) == cudaSuccess;
-  ok = ok && cudaMemsetAsync(p.hasprop, 0, L.cell - L.hasprop, s->stream) == cudaSuccess;
+  ok = ok && cudaMemsetAsync(p.hasprop, 0, L.partial - L.hasprop, s->stream) == cudaSuccess;   // proposal bits, both cell arrays
   ok = ok && cudaMemsetAsync(p.counts, 0, L.scal - L.counts, s->stream) == cudaSuccess;
   ok = ok && cudaMemcpyAsync(p.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream) == cudaSuccess;
   ok = ok && cudaMemcpyAsync((void*)p.tab, &T, sizeof(T), cudaMemcpyHostToDevice, s->stream) == cudaSuccess;
@@ -480,6 +494,9 @@ void sim_destroy(sim_t* s) {
     if (s->g8[k]) cudaGraphExecDestroy(s->g8[k]);
   }
   if (s->cap) cudaStreamDestroy(s->cap);
+  if (s->side) cudaStreamDestroy(s->side);
+  if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+  if (s->ev_join) cudaEventDestroy(s->ev_join);
   delete s;
 }
 
@@ -506,6 +523,7 @@ int sim_seed_population(sim_t* s, const sim_seed_rec_t* recs, uint32_t n_recs, u
   }
   CK(cudaGetLastError());
   sc.n_slots = dst; sc.next_id = id;
+  s->hist_valid = false;          // the population changed: the next step starts with the histogram prologue
   CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
   r = recount_row(s, sc.t, sc.n_slots);
   if (r) return r;
@@ -517,6 +535,7 @@ int sim_step_async(sim_t* s, uint32_t n_steps) {
   if (!s) return SIM_E_INVAL;
   if (s->sticky) return s->sticky;
   if ((uint64_t)s->t_host + n_steps >= s->cfg.counts_rows) return SIM_E_CAPACITY;
+  if (n_steps && !s->hist_valid) { int r = enqueue_prologue(s); if (r) return r; }
   if (!s->profile && !s->graphs_tried) build_graphs(s);
   uint32_t left = n_steps;
   if (!s->profile && s->graphs_ok) {
@@ -526,7 +545,7 @@ int sim_step_async(sim_t* s, uint32_t n_steps) {
     }
     while (left) {
       CK(cudaGraphLaunch(s->g1[parity_of(s)], s->stream));
-      std::swap(s->prm.cur, s->prm.oth);
+      flip(s);
       s->t_host++; s->launches += s->kernels_per_step; --left;
     }
     return SIM_OK;
@@ -644,7 +663,7 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
   sc.n_slots = n; sc.next_id = next_id; sc.t = step; sc.err = 0;
   sc.birth_count = sc.total_births = sc.ticket = 0;
   CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
-  s->t_host = step; s->sticky = SIM_OK;
+  s->t_host = step; s->sticky = SIM_OK; s->hist_valid = false;
   r = recount_row(s, step, n);   // also validates species / replica tile / id of every agent on the device
   if (r) return r;
   uint32_t err = 0;
@@ -663,9 +682,10 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
 
 int sim_debug_move_only(sim_t* s) {
   if (!s) return SIM_E_INVAL;
-  { ProfScope ps(s, KI_MOVE);
-    if (s->gauss_in_smem) k_move_only<true><<<s->grid_move, kMoveThreads, s->gauss_bytes, s->stream>>>(s->prm);
-    else k_move_only<false><<<s->grid_move, kMoveThreads, 0, s->stream>>>(s->prm); }
+  { ProfScope ps(s, KI_OTHER);
+    if (s->gauss_in_smem) k_move_only<true><<<s->grid_scatter, kMoveThreads, s->gauss_bytes, s->stream>>>(s->prm);
+    else k_move_only<false><<<s->grid_scatter, kMoveThreads, 0, s->stream>>>(s->prm); }
+  s->hist_valid = false;
   CK(cudaGetLastError());
   // crossing deltas went to row t+1: fold them back so that row t describes the moved state
   Scalars sc;
@@ -766,7 +786,7 @@ int sim_render(sim_t* s, const sim_view_t* view, uint8_t* rgba) {
   int r = read_scalars(s, &sc);
   if (r) return r;
   uint32_t* d_cnt = (uint32_t*)s->prm.birth_list;      // scratch that is free between steps
-  uchar4* d_img = (uchar4*)s->prm.off;
+  uchar4* d_img = (uchar4*)s->prm.prop;
   CK(cudaMemsetAsync(d_cnt, 0, n_pix * n_comp * 4, s->stream));
   if (sc.n_slots) {
     ProfScope ps(s, KI_OTHER);
