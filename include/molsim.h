@@ -129,10 +129,26 @@ int sim_read_agents(sim_t*, uint32_t cap, int32_t* x, int32_t* y, int32_t* z,
 
 /* Replaces the population by explicit agents in any order (checkpoint reload / test hook);
  * sets the step counter and next_id; rewrites counts row `step`.  HOST arrays (pinned memory makes
- * the copies asynchronous).  Species, replica tile (x >> stride_shift) and id < next_id of every
- * agent are validated on the device: on SIM_E_INVAL the handle holds an EMPTY population. */
+ * the copies asynchronous).  Every agent is validated on the device: species < n_species, replica tile
+ * (x >> stride_shift) < n_replicas, id < next_id and used once, and a position inside the compartment of its
+ * species (the invariant every step keeps, and what bounds the cell keys); on SIM_E_INVAL the handle holds an
+ * EMPTY population.  The delayed rules' t_first[] are left as they are (see sim_load_t_first). */
 int sim_load_agents(sim_t*, uint32_t n, const int32_t* x, const int32_t* y, const int32_t* z,
                     const uint16_t* species, const uint32_t* id, uint32_t step, uint32_t next_id);
+
+/* Order-independent 64-bit checksum of the live state: the sum, modulo 2^64, over live agents of
+ * mix(mix(mix(x | y << 32) ^ (z | id << 32)) ^ species) with mix = the splitmix64 finaliser (DESIGN.md §1
+ * "Checksum").  Computed on the device; *out is HOST.  It stands in for the element-by-element
+ * comparison at the sizes where the CPU oracle cannot be re-run inside a test (tests/golden/trace_*.txt).
+ * Synchronises the stream. */
+int sim_read_checksum(sim_t*, uint64_t* out);
+
+/* The part of a checkpoint that is not in the agents (state = agents, t, next_id, t_first[]): the
+ * first-firing step of every delayed rule (reading S17), 0xFFFFFFFF = not fired yet.  n must equal n_rules; HOST
+ * arrays.  sim_load_agents does not touch them: a reload that is to continue a run restores them with
+ * sim_load_t_first.  Both synchronise the stream. */
+int sim_read_t_first(sim_t*, uint32_t n, uint32_t* out);
+int sim_load_t_first(sim_t*, uint32_t n, const uint32_t* in);
 
 /* Current scalars (any pointer may be NULL).  Synchronises the stream. */
 int sim_info(sim_t*, uint32_t* n_live, uint32_t* step, uint32_t* next_id, uint32_t* t_first0);

@@ -70,6 +70,9 @@ def lib():
         L.oracle_read_agents.argtypes = [vp, u32, vp, vp, vp, vp, vp, P(u32)]
         L.oracle_load_agents.argtypes = [vp, u32, vp, vp, vp, vp, vp, u32, u32]
         L.oracle_info.argtypes = [vp, P(u32), P(u32), P(u32), P(u32)]
+        L.oracle_read_checksum.argtypes = [vp, P(u64)]
+        L.oracle_read_t_first.argtypes = [vp, u32, vp]
+        L.oracle_load_t_first.argtypes = [vp, u32, vp]
         L.oracle_philox4x32_10.argtypes = [vp, vp, vp]
         L.oracle_philox4x32_10.restype = None
         L.oracle_debug_move_only.argtypes = [vp]
@@ -191,6 +194,21 @@ class Oracle:
         if next_id is None:
             next_id = int(i.max()) + 1 if len(i) else 0
         _chk(lib().oracle_load_agents(self._h, len(x), _ptr(x), _ptr(y), _ptr(z), _ptr(s), _ptr(i), step, next_id))
+
+    def read_checksum(self):
+        v = C.c_uint64()
+        _chk(lib().oracle_read_checksum(self._h, C.byref(v)))
+        return v.value
+
+    def read_t_first(self):
+        out = np.zeros(max(1, self.model.n_rules), dtype=np.uint32)
+        if self.model.n_rules:
+            _chk(lib().oracle_read_t_first(self._h, self.model.n_rules, _ptr(out)))
+        return out[: self.model.n_rules]
+
+    def load_t_first(self, t_first):
+        a = np.ascontiguousarray(t_first, dtype=np.uint32)
+        _chk(lib().oracle_load_t_first(self._h, len(a), _ptr(a)))
 
     def debug_move_only(self):
         _chk(lib().oracle_debug_move_only(self._h))

@@ -502,6 +502,40 @@ int oracle_info(oracle_t* o, uint32_t* n_live, uint32_t* step, uint32_t* next_id
   return ORC_OK;
 }
 
+// Order-independent 64-bit checksum of the live state (DESIGN.md §1 "Checksum"):
+// sum over live agents, modulo 2^64, of h = mix(mix(mix(x | y << 32) ^ (z | id << 32)) ^ species) with the
+// coordinates taken as 32-bit patterns and mix = the splitmix64 finaliser written out below.
+static uint64_t mix64(uint64_t v) {
+  v ^= v >> 30; v *= 0xBF58476D1CE4E5B9ull;
+  v ^= v >> 27; v *= 0x94D049BB133111EBull;
+  v ^= v >> 31;
+  return v;
+}
+int oracle_read_checksum(oracle_t* o, uint64_t* out) {
+  if (!o || !out) return ORC_E_INVAL;
+  uint64_t sum = 0;
+  for (const Agent& a : o->ag) {
+    uint64_t lo = (uint64_t)(uint32_t)a.x | ((uint64_t)(uint32_t)a.y << 32);
+    uint64_t hi = (uint64_t)(uint32_t)a.z | ((uint64_t)a.id << 32);
+    sum += mix64(mix64(mix64(lo) ^ hi) ^ (uint64_t)a.s);
+  }
+  *out = sum;
+  return ORC_OK;
+}
+
+// Checkpoint state beyond the agents (state = agents, t, next_id, t_first[]): the first-firing
+// steps of the delayed rules (S17).  n must equal the model's n_rules.
+int oracle_read_t_first(oracle_t* o, uint32_t n, uint32_t* out) {
+  if (!o || !out || n != o->cfg.n_rules) return ORC_E_INVAL;
+  for (uint32_t r = 0; r < n; ++r) out[r] = o->t_first[r];
+  return ORC_OK;
+}
+int oracle_load_t_first(oracle_t* o, uint32_t n, const uint32_t* in) {
+  if (!o || !in || n != o->cfg.n_rules) return ORC_E_INVAL;
+  for (uint32_t r = 0; r < n; ++r) o->t_first[r] = in[r];
+  return ORC_OK;
+}
+
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) { philox(ctr, key, out); }
 
 int oracle_debug_move_only(oracle_t* o) { if (!o) return ORC_E_INVAL; o->phase_move(); return ORC_OK; }

@@ -75,6 +75,11 @@ int  oracle_read_agents(oracle_t*, uint32_t cap, int32_t* x, int32_t* y, int32_t
 int  oracle_load_agents(oracle_t*, uint32_t n, const int32_t* x, const int32_t* y, const int32_t* z,
                         const uint16_t* species, const uint32_t* id, uint32_t step, uint32_t next_id);
 int  oracle_info(oracle_t*, uint32_t* n_live, uint32_t* step, uint32_t* next_id, uint32_t* t_first0);
+/* order-independent 64-bit checksum of the live (id, species, x, y, z): DESIGN.md §1 "Checksum" */
+int  oracle_read_checksum(oracle_t*, uint64_t* out);
+/* first-firing steps of the delayed rules (S17), the part of a checkpoint that is not in the agents; n = n_rules */
+int  oracle_read_t_first(oracle_t*, uint32_t n, uint32_t* out);
+int  oracle_load_t_first(oracle_t*, uint32_t n, const uint32_t* in);
 
 /* test hooks */
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);

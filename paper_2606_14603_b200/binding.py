@@ -49,7 +49,8 @@ class _Config(C.Structure):
 EXPORTS = ["sim_workspace_bytes", "sim_create", "sim_seed_population", "sim_step", "sim_step_async",
            "sim_read_counts", "sim_read_agents", "sim_load_agents", "sim_info", "sim_debug_move_only",
            "sim_launch_count", "sim_profile_enable", "sim_kernel_times", "sim_kernel_name", "sim_destroy",
-           "sim_strerror", "sim_last_cuda_error", "sim_debug_philox", "sim_monitor_eval", "sim_render"]
+           "sim_strerror", "sim_last_cuda_error", "sim_debug_philox", "sim_monitor_eval", "sim_render",
+           "sim_read_checksum", "sim_read_t_first", "sim_load_t_first"]
 
 _lib = None
 
@@ -74,6 +75,9 @@ def load_library():
     L.sim_read_agents.argtypes = [vp, u32, vp, vp, vp, vp, vp, P(u32)]
     L.sim_load_agents.argtypes = [vp, u32, vp, vp, vp, vp, vp, u32, u32]
     L.sim_info.argtypes = [vp, P(u32), P(u32), P(u32), P(u32)]
+    L.sim_read_checksum.argtypes = [vp, P(C.c_uint64)]
+    L.sim_read_t_first.argtypes = [vp, u32, vp]
+    L.sim_load_t_first.argtypes = [vp, u32, vp]
     L.sim_debug_move_only.argtypes = [vp]
     L.sim_launch_count.argtypes = [vp]
     L.sim_launch_count.restype = C.c_uint64
@@ -237,6 +241,21 @@ class Sim:
             next_id = int(i.max()) + 1 if len(i) else 0
         self._check(self._lib.sim_load_agents(self._h, len(x), _ptr(x), _ptr(y), _ptr(z), _ptr(s), _ptr(i),
                                               step, next_id))
+
+    def read_checksum(self):
+        v = C.c_uint64()
+        self._check(self._lib.sim_read_checksum(self._h, C.byref(v)))
+        return v.value
+
+    def read_t_first(self):
+        out = np.zeros(max(1, self.model.n_rules), dtype=np.uint32)
+        if self.model.n_rules:
+            self._check(self._lib.sim_read_t_first(self._h, self.model.n_rules, _ptr(out)))
+        return out[: self.model.n_rules]
+
+    def load_t_first(self, t_first):
+        a = np.ascontiguousarray(t_first, dtype=np.uint32)
+        self._check(self._lib.sim_load_t_first(self._h, len(a), _ptr(a)))
 
     def debug_move_only(self):
         self._check(self._lib.sim_debug_move_only(self._h))

@@ -1017,21 +1017,35 @@ __global__ void k_seed(Params p, uint32_t species, uint32_t replica, uint32_t co
 }
 
 // Full histogram of the current state into counts row `r` (after seeding / loading), and its copy
-// into row r+1 as the base of the next step's deltas.
-__global__ void __launch_bounds__(256) k_count_row(Params p, uint32_t r, uint32_t n_slots) {
+// into row r+1 as the base of the next step's deltas.  With `check` (sim_load_agents: caller data) every agent is
+// validated as well: species, replica tile, id below next_id and not used twice (the id-indexed birth bitmap, all zero
+// between steps, serves as the "seen" set and is cleared again by k_clear_ids), and a position inside the compartment
+// of its species, which is what bounds every cell key the step computes.  A violation sets err bit 2.
+__global__ void __launch_bounds__(256) k_count_row(Params p, uint32_t r, uint32_t n_slots, bool check) {
   __shared__ int32_t s_delta[kMaxRowWidth];
   delta_zero(s_delta, p.row_width);
   const uint32_t next_id = p.scal->next_id;
+  const DevTables* __restrict__ T = p.tab;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += gridDim.x * blockDim.x) {
     const uint16_t s = p.cur.sp[i];
     if (s == kDead) continue;
     const int4 q = p.cur.r[i];
-    const uint32_t rep = (uint32_t)q.x >> p.stride_shift;
-    // sim_load_agents hands us caller data: species, replica tile and id are validated here (err bit 2)
-    if (s >= p.n_species || rep >= p.n_replicas || (uint32_t)q.w >= next_id) { atomicOr(&p.scal->err, 4u); continue; }
+    const uint32_t rep = (uint32_t)q.x >> p.stride_shift, id = (uint32_t)q.w;
+    if (check) {
+      bool ok = q.x >= 0 && s < p.n_species && rep < p.n_replicas && id < next_id;
+      if (ok) ok = comp_valid(T->comp[T->sp[s].compartment], q.x - (int32_t)(rep << p.stride_shift), q.y, q.z);
+      if (ok) ok = !(atomicOr(&p.bits[id >> 3], 1u << ((id & 7u) * 4u)) >> ((id & 7u) * 4u) & 1u);
+      if (!ok) { atomicOr(&p.scal->err, 4u); continue; }
+    }
     atomicAdd(&s_delta[rep * p.n_species + s], 1);
   }
   delta_flush(s_delta, p.counts + (size_t)r * p.row_width, p.row_width);
+}
+__global__ void __launch_bounds__(256) k_clear_ids(Params p, uint32_t n_slots) {
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += gridDim.x * blockDim.x) {
+    const uint32_t id = (uint32_t)p.cur.r[i].w;
+    if (id < p.id_capacity) p.bits[id >> 3] = 0u;
+  }
 }
 __global__ void k_copy_row(Params p, uint32_t r) {
   const uint32_t* src = p.counts + (size_t)r * p.row_width;

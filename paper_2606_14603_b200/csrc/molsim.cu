@@ -213,11 +213,12 @@ int err_from_bits(uint32_t bits) {
 }
 
 // counts row r <- histogram of the current state; row r+1 <- copy (base of the next step's deltas)
-int recount_row(sim* s, uint32_t r, uint32_t n_slots) {
+int recount_row(sim* s, uint32_t r, uint32_t n_slots, bool check = false) {
   CK(cudaMemsetAsync(s->prm.counts + (size_t)r * s->prm.row_width, 0, (size_t)s->prm.row_width * 4, s->stream));
   if (n_slots) {
     ProfScope ps(s, KI_OTHER);
-    k_count_row<<<std::min<uint32_t>((n_slots + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, r, n_slots);
+    k_count_row<<<std::min<uint32_t>((n_slots + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, r, n_slots, check);
+    if (check) k_clear_ids<<<std::min<uint32_t>((n_slots + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, n_slots);
   }
   { ProfScope ps(s, KI_OTHER); k_copy_row<<<1, 256, 0, s->stream>>>(s->prm, r); }
   CK(cudaGetLastError());
@@ -664,7 +665,7 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
   sc.birth_count = sc.total_births = sc.ticket = 0;
   CK(cudaMemcpyAsync(s->prm.scal, &sc, sizeof(sc), cudaMemcpyHostToDevice, s->stream));
   s->t_host = step; s->sticky = SIM_OK; s->hist_valid = false;
-  r = recount_row(s, step, n);   // also validates species / replica tile / id of every agent on the device
+  r = recount_row(s, step, n, true);   // also validates every agent on the device (k_count_row)
   if (r) return r;
   uint32_t err = 0;
   CK(cudaMemcpyAsync(&err, &s->prm.scal->err, 4, cudaMemcpyDeviceToHost, s->stream));
@@ -677,6 +678,41 @@ int sim_load_agents(sim_t* s, uint32_t n, const int32_t* x, const int32_t* y, co
     CK(cudaStreamSynchronize(s->stream));
     return SIM_E_INVAL;
   }
+  return SIM_OK;
+}
+
+int sim_read_checksum(sim_t* s, uint64_t* out) {
+  if (!s || !out) return SIM_E_INVAL;
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  unsigned long long* d_sum = (unsigned long long*)s->prm.birth_list;     // scratch that is free between steps
+  CK(cudaMemsetAsync(d_sum, 0, 8, s->stream));
+  if (sc.n_slots) {
+    ProfScope ps(s, KI_OTHER);
+    k_checksum<<<std::min<uint32_t>((sc.n_slots + 255) / 256, 148 * 8), 256, 0, s->stream>>>(s->prm, sc.n_slots, d_sum);
+  }
+  CK(cudaGetLastError());
+  unsigned long long h = 0;
+  CK(cudaMemcpyAsync(&h, d_sum, 8, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  *out = h;
+  return SIM_OK;
+}
+
+int sim_read_t_first(sim_t* s, uint32_t n, uint32_t* out) {
+  if (!s || !out || n != s->cfg.n_rules) return SIM_E_INVAL;
+  Scalars sc;
+  int r = read_scalars(s, &sc);
+  if (r) return r;
+  for (uint32_t k = 0; k < n; ++k) out[k] = sc.t_first[k];
+  return SIM_OK;
+}
+
+int sim_load_t_first(sim_t* s, uint32_t n, const uint32_t* in) {
+  if (!s || !in || n != s->cfg.n_rules) return SIM_E_INVAL;
+  if (n) CK(cudaMemcpyAsync(s->prm.scal->t_first, in, (size_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
   return SIM_OK;
 }
 

@@ -5,6 +5,32 @@
 
 namespace molsim {
 
+// ----------------------------------------------------------------------------- state checksum
+// Order-independent 64-bit checksum of the live state (DESIGN.md §1 "Checksum"): the sum, modulo 2^64, over live
+// agents of mix(mix(mix(x | y << 32) ^ (z | id << 32)) ^ species), coordinates as 32-bit patterns, mix = the
+// splitmix64 finaliser.  A sum, so the slot order the sort leaves behind does not matter.  This is what lets the
+// full-size runs the CPU oracle cannot repeat inside a test be compared step by step (tests/golden/trace_*.txt).
+__device__ __forceinline__ unsigned long long mix64(unsigned long long v) {
+  v ^= v >> 30; v *= 0xBF58476D1CE4E5B9ull;
+  v ^= v >> 27; v *= 0x94D049BB133111EBull;
+  v ^= v >> 31;
+  return v;
+}
+__global__ void __launch_bounds__(256) k_checksum(Params p, uint32_t n_slots, unsigned long long* __restrict__ out) {
+  unsigned long long sum = 0;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += gridDim.x * blockDim.x) {
+    const uint16_t s = p.cur.sp[i];
+    if (s == kDead) continue;
+    const int4 q = p.cur.r[i];
+    const unsigned long long lo = (unsigned long long)(uint32_t)q.x | ((unsigned long long)(uint32_t)q.y << 32);
+    const unsigned long long hi = (unsigned long long)(uint32_t)q.z | ((unsigned long long)(uint32_t)q.w << 32);
+    sum += mix64(mix64(mix64(lo) ^ hi) ^ (unsigned long long)s);
+  }
+#pragma unroll
+  for (int d = 16; d; d >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, d);
+  if ((threadIdx.x & 31u) == 0u && sum) atomicAdd(out, sum);
+}
+
 // ----------------------------------------------------------------------------- N3 threshold monitor
 // One block per monitor; threads stride over the rows of the window, then a block reduction.
 // Everything is integer and order-free (min / max / sum), so the result is unique (reading S24).
