@@ -31,11 +31,12 @@ CASES = {
     "w4_64m": (lambda: configs.w4(n=64_000_000, n_steps=1), 1, "[CFG 4] N = 64 M, scaling claim PAPER.md:107"),
     "w1_full": (lambda: configs.w1(n_steps=200), 200, "[CFG 1] full size (MAPK-shaped cascade, PAPER.md:80-97)"),
     "w2_full": (lambda: configs.w2(n_steps=20), 20, "[CFG 2] full size, 8 replicas (dose sweep, PAPER.md:80-82)"),
-    "w3_full": (lambda: configs.w3(n_steps=W3_STEPS, delay=W3_DELAY), None,
-                "[CFG 3] full size with the repressor delay shortened to W3_DELAY steps so that the delayed rule fires "
-                "inside the trace (cFos expression, PAPER.md:153-167)"),
+    "w3_full": (lambda: configs.w3(**W3_TRACE), None,
+                "[CFG 3] full size, with a 50 nm gene locus, 2,000 nuclear pERK seeded at t = 0 and the repressor delay "
+                "shortened to 200 steps so that transcription, export, translation and the delayed rule all happen "
+                "inside the trace (cFos expression, PAPER.md:153-167; workloads/configs.py w3)"),
 }
-W3_STEPS, W3_DELAY = 1400, 200
+W3_TRACE = dict(n_steps=800, delay=200, gene_radius=500, primed_perk_n=2000)
 
 
 def run(case):

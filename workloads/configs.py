@@ -148,8 +148,15 @@ def w2(scale: float = 1.0, n_steps: int = 5_000, cell_size: int = 1024, seed: in
 
 # ----------------------------------------------------------------------------- W3
 def w3(scale: float = 1.0, n_steps: int = 20_000, cell_size: int = 1024, seed: int = 4,
-       delay: int = 2_000) -> Model:
-    """[CFG 3]: cytoplasm shell + nucleus, membrane crossing, expression, delayed repressor."""
+       delay: int = 2_000, gene_radius: int = R_BIND, primed_perk_n: int = 0) -> Model:
+    """[CFG 3]: cytoplasm shell + nucleus, membrane crossing, expression, delayed repressor.
+
+    `gene_radius` (units) is the capture radius of the two gene-locus agents for nuclear pERK and for the repressor.
+    [CFG 3] gives none; reading S18 takes the 5 nm of the other reactions, with which a full-size run practically never
+    transcribes (a few dozen nuclear pERK against two 5 nm targets in 65 um^3).  The long-run parity trace
+    (tests/golden/make_traces.py) therefore uses a 50 nm locus, `primed_perk_n` nuclear pERK seeded at t = 0 and a
+    200-step delay, so that the expression branch and the delayed rule run at full size inside a trace the oracle can
+    produce; parity does not depend on the values."""
     CYT, NUC = 0, 1
     sp, rx, ix = _cascade_species(comp=CYT)
 
@@ -194,14 +201,16 @@ def w3(scale: float = 1.0, n_steps: int = 20_000, cell_size: int = 1024, seed: i
         _release(p_rel, GENE, pERK_n),
         emit_F,
     ]
-    rx.append(Reaction(GENE, pERK_n, GENE_pERK, R2_BIND, prob_to_thr(0.5)))
-    rx.append(Reaction(GENE, F_n, GENE_F, R2_BIND, prob_to_thr(0.5)))
+    rx.append(Reaction(GENE, pERK_n, GENE_pERK, gene_radius * gene_radius, prob_to_thr(0.5)))
+    rx.append(Reaction(GENE, F_n, GENE_F, gene_radius * gene_radius, prob_to_thr(0.5)))
 
     R = int(round(SPHERE_R * scale ** (1.0 / 3.0)))
     Rn = R // 2
     counts = [("BRAF", 12_500), ("MEK", 75_000), ("ERK", 150_000), ("P", 25_000), ("RSK", 75_000)]
     recs = [SeedRecord(ix[n], max(1, int(round(c * scale)))) for n, c in counts]
     recs.append(SeedRecord(GENE, 2))
+    if primed_perk_n:
+        recs.append(SeedRecord(pERK_n, primed_perk_n))
     m = Model(
         name="W3_nuclear", species=sp, reactions=rx,
         compartments=[Compartment(SHAPE_SPHERE, R, R, R, r_out=R, r_in=Rn),
