@@ -94,6 +94,30 @@ typedef struct {
 
 typedef struct sim sim_t;   /* opaque; owned by the library, freed by sim_destroy */
 
+/* Table validation (the in-scope part of the paper's consistency checker, plus the bounds the kernels rely
+ * on).  sim_workspace_bytes / sim_create fail with 0 / SIM_E_INVAL unless ALL of these hold:
+ *  V1  species, compartments, tables (and reactions when n_reactions > 0) are given.
+ *  V2  1 <= n_species <= SIM_MAX_SPECIES, n_reactions <= SIM_MAX_REACTIONS, 1 <= n_compartments <= SIM_MAX_COMPARTMENTS,
+ *      n_rules <= SIM_MAX_RULES, 1 <= table_bits <= 16, 1 <= n_sigma_classes <= 255, 1 <= n_replicas <= SIM_MAX_REPLICAS,
+ *      stride_shift <= 31, 2 <= cell_size <= 16384, 1 <= capacity < 2^31, id_capacity >= 1, counts_rows >= 1, extent > 0.
+ *  V3  the replica tiles fit int32 (n_replicas << stride_shift <= 2^31 when n_replicas > 1) and cover extent[0].
+ *  V4  every compartment is well formed (cube: L > 0 and every displacement table entry of a mobile class is smaller than
+ *      L in magnitude, so that one mirror reflection suffices, S5; sphere: 0 < r_out, r_in < r_out), its bounding box lies
+ *      inside [0, extent) in y and z and inside [0, tile) in x (tile = extent[0], or 2^stride_shift with replicas), and with
+ *      replicas its upper x bound stays at least the largest interaction radius below the tile width, so that agents of
+ *      neighbouring replicas can never bind (S16: replicas are independent populations).
+ *  V5  every species names an existing sigma class and compartment, has at most SIM_MAX_CHANNELS channels, and its
+ *      cross_to, if any, is a species of ANOTHER compartment, both spherical (S7).
+ *  V6  every channel has a known kind; the products it needs exist and live in the parent's compartment (prod0: RELEASE,
+ *      CONVERT; prod1: RELEASE, BIRTH, DELAYED_BIRTH: "references to undefined species"); a rule slot it
+ *      uses is below n_rules; a DELAYED_BIRTH delay is at least one step (S17).
+ *  V7  every reaction names existing species that share a compartment with their complex, its radius fits the cell
+ *      (r2 <= cell_size^2: the 27-cell search is exact, S8), and no unordered species pair has two reactions (the
+ *      paper's "reciprocal reactions" are ONE symmetric entry here).
+ * sim_check_config returns NULL when the configuration is valid, else a static string that names the first rule
+ * that fails (host only; needs no device). */
+const char* sim_check_config(const sim_config_t* cfg);
+
 /* Bytes of DEVICE workspace sim_create needs for this configuration (0 if cfg is invalid). */
 size_t sim_workspace_bytes(const sim_config_t* cfg);
 

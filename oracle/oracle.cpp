@@ -318,6 +318,12 @@ static int validate(const orc_config_t* c) {
   int32_t max_tab = 0;
   for (size_t i = (size_t)1 << c->table_bits; i < ((size_t)c->n_sigma_classes << c->table_bits); ++i)
     max_tab = std::max<int32_t>(max_tab, std::abs((int32_t)c->tables[i]));
+  // DESIGN.md S16: replicas are independent populations, so with several of them a compartment must end at least the
+  // largest interaction radius (ceil sqrt max r2) before the next tile begins
+  int64_t max_r = 0;
+  if (c->reactions)
+    for (uint32_t e = 0; e < c->n_reactions; ++e)
+      while (max_r * max_r < (int64_t)c->reactions[e].r2) ++max_r;
   for (uint32_t i = 0; i < c->n_compartments; ++i) {
     const orc_compartment_t& k = c->compartments[i];
     int64_t hi;
@@ -330,7 +336,7 @@ static int validate(const orc_config_t* c) {
     } else return ORC_E_INVAL;
     if (k.shape == ORC_SHAPE_CUBE && (k.L > c->extent[1] || k.L > c->extent[2])) return ORC_E_INVAL;
     if (c->n_replicas == 1 && hi > c->extent[0]) return ORC_E_INVAL;
-    if (c->n_replicas > 1 && hi > ((int64_t)1 << c->stride_shift)) return ORC_E_INVAL;
+    if (c->n_replicas > 1 && hi + max_r > ((int64_t)1 << c->stride_shift)) return ORC_E_INVAL;
   }
   for (uint32_t i = 0; i < c->n_species; ++i) {
     const orc_species_t& s = c->species[i];

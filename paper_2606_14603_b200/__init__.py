@@ -5,4 +5,4 @@ marshalling only; every step of the path runs in the hand-written sm_100a kernel
 used for device memory and the stream.  There is no CPU fallback: loading fails loudly when the
 library has not been built.
 """
-from .binding import Sim, SimError, load_library  # noqa: F401
+from .binding import Sim, SimError, check_config, load_library  # noqa: F401

@@ -50,7 +50,7 @@ EXPORTS = ["sim_workspace_bytes", "sim_create", "sim_seed_population", "sim_step
            "sim_read_counts", "sim_read_agents", "sim_load_agents", "sim_info", "sim_debug_move_only",
            "sim_launch_count", "sim_profile_enable", "sim_kernel_times", "sim_kernel_name", "sim_destroy",
            "sim_strerror", "sim_last_cuda_error", "sim_debug_philox", "sim_monitor_eval", "sim_render",
-           "sim_read_checksum", "sim_read_t_first", "sim_load_t_first"]
+           "sim_read_checksum", "sim_read_t_first", "sim_load_t_first", "sim_check_config"]
 
 _lib = None
 
@@ -78,6 +78,8 @@ def load_library():
     L.sim_read_checksum.argtypes = [vp, P(C.c_uint64)]
     L.sim_read_t_first.argtypes = [vp, u32, vp]
     L.sim_load_t_first.argtypes = [vp, u32, vp]
+    L.sim_check_config.argtypes = [P(_Config)]
+    L.sim_check_config.restype = C.c_char_p
     L.sim_debug_move_only.argtypes = [vp]
     L.sim_launch_count.argtypes = [vp]
     L.sim_launch_count.restype = C.c_uint64
@@ -156,6 +158,13 @@ def marshal_config(m, cell_size=None, seed=None):
     return cfg, (sp, rx, cp, tab)
 
 
+def check_config(model, cell_size=None):
+    """sim_check_config: None when the tables are valid, else the name of the first rule (V1-V7) that fails.  Host only."""
+    cfg, keep = marshal_config(model, cell_size, None)
+    why = load_library().sim_check_config(C.byref(cfg))
+    return None if why is None else why.decode()
+
+
 class Sim:
     """One population on one GPU.  Methods mirror the C ABI one to one."""
 
@@ -167,7 +176,8 @@ class Sim:
         cfg, keep = marshal_config(model, cell_size, seed)
         nbytes = self._lib.sim_workspace_bytes(C.byref(cfg))
         if nbytes == 0:
-            raise SimError(E_INVAL, "(sim_workspace_bytes)")
+            why = self._lib.sim_check_config(C.byref(cfg))
+            raise SimError(E_INVAL, f"(sim_workspace_bytes: {why.decode() if why else 'cell grid too large'})")
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)

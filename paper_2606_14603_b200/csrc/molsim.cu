@@ -64,75 +64,141 @@ bool make_layout(const sim_config_t* c, Layout& L) {
   return true;
 }
 
-// Table validation: the in-scope part of the paper's consistency checker plus the
-// bounds the kernels rely on.
-int validate(const sim_config_t* c) {
-  if (!c || !c->species || !c->compartments || !c->tables) return SIM_E_INVAL;
-  if (c->n_reactions && !c->reactions) return SIM_E_INVAL;
-  if (c->n_species == 0 || c->n_species > SIM_MAX_SPECIES || c->n_reactions > SIM_MAX_REACTIONS) return SIM_E_INVAL;
-  if (c->n_compartments == 0 || c->n_compartments > SIM_MAX_COMPARTMENTS || c->n_rules > SIM_MAX_RULES) return SIM_E_INVAL;
-  if (c->table_bits < 1 || c->table_bits > 16 || c->n_sigma_classes < 1 || c->n_sigma_classes > 255) return SIM_E_INVAL;
-  if (c->n_replicas < 1 || c->n_replicas > SIM_MAX_REPLICAS || c->stride_shift > 31) return SIM_E_INVAL;
-  if (c->cell_size < 2 || c->cell_size > 16384) return SIM_E_INVAL;
-  if (c->capacity == 0 || c->capacity > 0x7FFFFFFFu || c->counts_rows == 0 || c->id_capacity == 0) return SIM_E_INVAL;
-  for (int a = 0; a < 3; ++a) if (c->extent[a] <= 0) return SIM_E_INVAL;
-  if (c->n_replicas > 1 && ((uint64_t)c->n_replicas << c->stride_shift) > 0x80000000ull) return SIM_E_INVAL;
-  if ((uint64_t)c->extent[0] > ((uint64_t)c->n_replicas << c->stride_shift)) return SIM_E_INVAL;
-  int32_t max_tab = 0;
-  for (size_t i = (size_t)1 << c->table_bits; i < ((size_t)c->n_sigma_classes << c->table_bits); ++i)
-    max_tab = std::max<int32_t>(max_tab, std::abs((int32_t)c->tables[i]));
-  for (uint32_t i = 0; i < c->n_compartments; ++i) {
-    const sim_compartment_t& k = c->compartments[i];
-    int64_t hi_x;
-    if (k.shape == SIM_SHAPE_CUBE) {
-      if (k.L <= 0 || max_tab >= k.L || k.L > c->extent[1] || k.L > c->extent[2]) return SIM_E_INVAL;
-      hi_x = k.L;
-    } else if (k.shape == SIM_SHAPE_SPHERE) {
-      if (k.r_out <= 0 || k.r_in >= k.r_out) return SIM_E_INVAL;
-      if (k.cx - k.r_out < 0 || k.cy - k.r_out < 0 || k.cz - k.r_out < 0) return SIM_E_INVAL;
-      if ((int64_t)k.cy + k.r_out >= c->extent[1] || (int64_t)k.cz + k.r_out >= c->extent[2]) return SIM_E_INVAL;
-      hi_x = (int64_t)k.cx + k.r_out + 1;
-    } else {
-      return SIM_E_INVAL;
-    }
-    if (c->n_replicas > 1 && hi_x > ((int64_t)1 << c->stride_shift)) return SIM_E_INVAL;
-    if (c->n_replicas == 1 && hi_x > c->extent[0]) return SIM_E_INVAL;
+// Table validation: the in-scope part of the paper's consistency checker ("missing reciprocal
+// reactions, references to undefined species ... inconsistencies between specified volume and concentration") plus
+// the bounds the kernels rely on.  Written from the rule list in include/molsim.h ("Table validation", V1-V7), rule
+// by rule; returns the name of the first rule that fails, or nullptr.  tests/test_validation_rules.py states every
+// rule and checks that this checker and the oracle's (written from DESIGN.md, separately) both enforce it.
+struct ConfigCheck {
+  const sim_config_t& c;
+  explicit ConfigCheck(const sim_config_t& cfg) : c(cfg) {}
+
+  // largest displacement of any mobile class, and the largest interaction radius (ceil sqrt of the largest r2)
+  int64_t max_step() const {
+    int64_t m = 0;
+    const size_t n = (size_t)1 << c.table_bits;
+    for (uint32_t cls = 1; cls < c.n_sigma_classes; ++cls)
+      for (size_t k = 0; k < n; ++k) m = std::max<int64_t>(m, std::llabs((long long)c.tables[cls * n + k]));
+    return m;
   }
-  for (uint32_t i = 0; i < c->n_species; ++i) {
-    const sim_species_t& s = c->species[i];
-    if (s.sigma_class >= c->n_sigma_classes || s.compartment >= c->n_compartments) return SIM_E_INVAL;
-    if (s.n_channels > SIM_MAX_CHANNELS) return SIM_E_INVAL;
-    if (s.cross_to != SIM_NONE16) {
-      if (s.cross_to >= c->n_species) return SIM_E_INVAL;
-      const uint32_t oc = c->species[s.cross_to].compartment;
-      if (oc == s.compartment) return SIM_E_INVAL;
-      if (c->compartments[oc].shape == SIM_SHAPE_CUBE || c->compartments[s.compartment].shape == SIM_SHAPE_CUBE)
-        return SIM_E_INVAL;
-    }
-    for (uint32_t k = 0; k < s.n_channels; ++k) {
-      const sim_channel_t& ch = s.ch[k];
-      if (ch.kind > SIM_CH_DELAYED_BIRTH) return SIM_E_INVAL;
-      const bool needs0 = ch.kind == SIM_CH_RELEASE || ch.kind == SIM_CH_CONVERT;
-      const bool needs1 = ch.kind == SIM_CH_RELEASE || ch.kind == SIM_CH_BIRTH || ch.kind == SIM_CH_DELAYED_BIRTH;
-      if (needs0 && (ch.prod0 >= c->n_species || c->species[ch.prod0].compartment != s.compartment)) return SIM_E_INVAL;
-      if (needs1 && (ch.prod1 >= c->n_species || c->species[ch.prod1].compartment != s.compartment)) return SIM_E_INVAL;
-      if ((ch.kind == SIM_CH_DELAYED_BIRTH || ch.marks_first) && ch.rule >= c->n_rules) return SIM_E_INVAL;
-      if (ch.kind == SIM_CH_DELAYED_BIRTH && ch.thr < 1) return SIM_E_INVAL;
-    }
+  int64_t max_radius() const {
+    uint64_t r2 = 0;
+    for (uint32_t e = 0; e < c.n_reactions; ++e) r2 = std::max<uint64_t>(r2, c.reactions[e].r2);
+    int64_t r = (int64_t)std::sqrt((double)r2);
+    while ((uint64_t)r * (uint64_t)r < r2) ++r;
+    while (r > 0 && (uint64_t)(r - 1) * (uint64_t)(r - 1) >= r2) --r;
+    return r;
   }
-  for (uint32_t e = 0; e < c->n_reactions; ++e) {
-    const sim_reaction_t& r = c->reactions[e];
-    if (r.a >= c->n_species || r.b >= c->n_species || r.cplx >= c->n_species) return SIM_E_INVAL;
-    const uint32_t ca = c->species[r.a].compartment;
-    if (c->species[r.b].compartment != ca || c->species[r.cplx].compartment != ca) return SIM_E_INVAL;
-    if ((uint64_t)r.r2 > (uint64_t)c->cell_size * c->cell_size) return SIM_E_INVAL;
-    for (uint32_t f = 0; f < e; ++f) {
-      const sim_reaction_t& q = c->reactions[f];
-      if ((q.a == r.a && q.b == r.b) || (q.a == r.b && q.b == r.a)) return SIM_E_INVAL;
-    }
+  int64_t tile_width() const { return c.n_replicas > 1 ? ((int64_t)1 << c.stride_shift) : (int64_t)c.extent[0]; }
+  bool species_ok(uint32_t s) const { return s < c.n_species; }
+  bool same_compartment(uint32_t s, uint32_t other) const {
+    return species_ok(other) && c.species[other].compartment == c.species[s].compartment;
   }
-  return SIM_OK;
-}
+
+  const char* limits() const {                                                    // V1, V2
+    if (!c.species || !c.compartments || !c.tables || (c.n_reactions && !c.reactions)) return "V1 table pointer missing";
+    if (c.n_species < 1 || c.n_species > SIM_MAX_SPECIES) return "V2 n_species outside 1..SIM_MAX_SPECIES";
+    if (c.n_reactions > SIM_MAX_REACTIONS) return "V2 n_reactions above SIM_MAX_REACTIONS";
+    if (c.n_compartments < 1 || c.n_compartments > SIM_MAX_COMPARTMENTS) return "V2 n_compartments outside 1..SIM_MAX_COMPARTMENTS";
+    if (c.n_rules > SIM_MAX_RULES) return "V2 n_rules above SIM_MAX_RULES";
+    if (c.table_bits < 1 || c.table_bits > 16) return "V2 table_bits outside 1..16";
+    if (c.n_sigma_classes < 1 || c.n_sigma_classes > 255) return "V2 n_sigma_classes outside 1..255";
+    if (c.n_replicas < 1 || c.n_replicas > SIM_MAX_REPLICAS || c.stride_shift > 31) return "V2 replica tiling outside its limits";
+    if (c.cell_size < 2 || c.cell_size > 16384) return "V2 cell_size outside 2..16384";
+    if (c.capacity < 1 || c.capacity > 0x7FFFFFFFu || c.id_capacity < 1 || c.counts_rows < 1) return "V2 capacity / id_capacity / counts_rows";
+    for (int a = 0; a < 3; ++a) if (c.extent[a] <= 0) return "V2 extent not positive";
+    return nullptr;
+  }
+  const char* tiling() const {                                                    // V3
+    const uint64_t span = (uint64_t)c.n_replicas << c.stride_shift;
+    if (c.n_replicas > 1 && span > 0x80000000ull) return "V3 replica tiles do not fit int32";
+    if ((uint64_t)c.extent[0] > span) return "V3 extent[0] wider than the replica tiles";
+    return nullptr;
+  }
+  const char* geometry() const {                                                  // V4
+    const int64_t step = max_step(), reach = max_radius(), tile = tile_width();
+    for (uint32_t k = 0; k < c.n_compartments; ++k) {
+      const sim_compartment_t& g = c.compartments[k];
+      int64_t lo[3], hi[3];                       // bounding box in local coordinates, hi exclusive
+      if (g.shape == SIM_SHAPE_CUBE) {
+        if (g.L <= 0) return "V4 cube edge not positive";
+        if (step >= g.L) return "V4 a displacement table entry reaches across the cube (one mirror reflection must suffice)";
+        for (int a = 0; a < 3; ++a) { lo[a] = 0; hi[a] = g.L; }
+      } else if (g.shape == SIM_SHAPE_SPHERE) {
+        if (g.r_out <= 0 || g.r_in >= g.r_out) return "V4 sphere radii (need 0 < r_out and r_in < r_out)";
+        const int64_t ctr[3] = {g.cx, g.cy, g.cz};
+        for (int a = 0; a < 3; ++a) { lo[a] = ctr[a] - g.r_out; hi[a] = ctr[a] + g.r_out + 1; }
+      } else {
+        return "V4 unknown compartment shape";
+      }
+      if (lo[0] < 0 || lo[1] < 0 || lo[2] < 0) return "V4 compartment reaches below 0";
+      if (hi[1] > c.extent[1] || hi[2] > c.extent[2]) return "V4 compartment reaches beyond extent (y / z)";
+      if (hi[0] > tile) return "V4 compartment reaches beyond its tile / extent (x)";
+      if (c.n_replicas > 1 && hi[0] + reach > tile) return "V4 replicas closer than the largest interaction radius";
+    }
+    return nullptr;
+  }
+  const char* species() const {                                                   // V5, V6
+    for (uint32_t s = 0; s < c.n_species; ++s) {
+      const sim_species_t& sp = c.species[s];
+      if (sp.sigma_class >= c.n_sigma_classes) return "V5 sigma_class out of range";
+      if (sp.compartment >= c.n_compartments) return "V5 compartment out of range";
+      if (sp.n_channels > SIM_MAX_CHANNELS) return "V5 more than SIM_MAX_CHANNELS channels";
+      if (sp.cross_to != SIM_NONE16) {
+        if (!species_ok(sp.cross_to)) return "V5 cross_to is not a species";
+        const uint32_t there = c.species[sp.cross_to].compartment;
+        if (there >= c.n_compartments || there == sp.compartment) return "V5 cross_to lives in the same compartment";
+        if (c.compartments[there].shape != SIM_SHAPE_SPHERE || c.compartments[sp.compartment].shape != SIM_SHAPE_SPHERE)
+          return "V5 membrane crossing needs spherical compartments";
+      }
+      for (uint32_t k = 0; k < sp.n_channels; ++k) {
+        const sim_channel_t& ch = sp.ch[k];
+        switch (ch.kind) {
+          case SIM_CH_NONE: case SIM_CH_DEGRADE: break;
+          case SIM_CH_CONVERT:
+            if (!same_compartment(s, ch.prod0)) return "V6 product 0 missing or in another compartment";
+            break;
+          case SIM_CH_RELEASE:
+            if (!same_compartment(s, ch.prod0)) return "V6 product 0 missing or in another compartment";
+            if (!same_compartment(s, ch.prod1)) return "V6 product 1 missing or in another compartment";
+            break;
+          case SIM_CH_BIRTH: case SIM_CH_DELAYED_BIRTH:
+            if (!same_compartment(s, ch.prod1)) return "V6 product 1 missing or in another compartment";
+            break;
+          default: return "V6 unknown channel kind";
+        }
+        if ((ch.kind == SIM_CH_DELAYED_BIRTH || ch.marks_first) && ch.rule >= c.n_rules) return "V6 rule slot out of range";
+        if (ch.kind == SIM_CH_DELAYED_BIRTH && ch.thr < 1) return "V6 delay of a delayed birth below one step";
+      }
+    }
+    return nullptr;
+  }
+  const char* reactions() const {                                                 // V7
+    const uint64_t cell2 = (uint64_t)c.cell_size * c.cell_size;
+    std::vector<uint8_t> seen((size_t)c.n_species * c.n_species, 0);
+    for (uint32_t e = 0; e < c.n_reactions; ++e) {
+      const sim_reaction_t& r = c.reactions[e];
+      if (!species_ok(r.a) || !species_ok(r.b) || !species_ok(r.cplx)) return "V7 reaction names an undefined species";
+      if (!same_compartment(r.a, r.b) || !same_compartment(r.a, r.cplx)) return "V7 reactants and complex in different compartments";
+      if ((uint64_t)r.r2 > cell2) return "V7 interaction radius above the cell size";
+      uint8_t& ab = seen[(size_t)std::min(r.a, r.b) * c.n_species + std::max(r.a, r.b)];
+      if (ab) return "V7 two reactions for the same pair of species";
+      ab = 1;
+    }
+    return nullptr;
+  }
+  const char* run() const {
+    const char* why = limits();
+    if (!why) why = tiling();
+    if (!why) why = species();
+    if (!why) why = reactions();
+    if (!why) why = geometry();
+    return why;
+  }
+};
+
+const char* check_config(const sim_config_t* c) { return c ? ConfigCheck(*c).run() : "V1 no configuration"; }
+int validate(const sim_config_t* c) { return check_config(c) ? SIM_E_INVAL : SIM_OK; }
 
 }  // namespace
 
@@ -767,6 +833,8 @@ const char* sim_strerror(int code) {
 }
 
 const char* sim_last_cuda_error(const sim_t* s) { return s ? s->cuda_err.c_str() : ""; }
+
+const char* sim_check_config(const sim_config_t* cfg) { return check_config(cfg); }
 
 int sim_monitor_eval(sim_t* s, const sim_monitor_t* mons, uint32_t n_mons, sim_monitor_result_t* out,
                      uint8_t* states, uint32_t states_stride) {
