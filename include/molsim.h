@@ -31,7 +31,8 @@ enum { SIM_OK = 0,
        SIM_E_INVAL = -1,     /* table validation failed / bad argument (cf. the paper's consistency checker) */
        SIM_E_CAPACITY = -2,  /* agent slots, counts rows or an output buffer too small */
        SIM_E_IDSPACE = -3,   /* next_id would pass id_capacity */
-       SIM_E_CUDA = -4 };    /* CUDA runtime error (sim_last_cuda_error has the text) */
+       SIM_E_CUDA = -4,      /* CUDA runtime error (sim_last_cuda_error has the text) */
+       SIM_E_INTERNAL = -5 };/* checked build only (-DMOLSIM_CHECKS): an index a kernel derived from data left its bound */
 
 /* unimolecular channel kinds — DESIGN.md §1 phase 3 */
 enum { SIM_CH_NONE = 0, SIM_CH_BIRTH = 1, SIM_CH_RELEASE = 2, SIM_CH_CONVERT = 3,

@@ -3,7 +3,10 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB = os.path.join(HERE, "liboracle.so")
+# ORACLE_SANITIZE=1: AddressSanitizer + UndefinedBehaviorSanitizer build (run the CPU tests with
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0; profiles/r2_sanitizers.md)
+SANITIZE = os.environ.get("ORACLE_SANITIZE") == "1"
+LIB = os.path.join(HERE, "liboracle_san.so" if SANITIZE else "liboracle.so")
 
 
 def build(force: bool = False) -> str:
@@ -12,6 +15,8 @@ def build(force: bool = False) -> str:
         return LIB
     cmd = ["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-Wall", "-Wno-misleading-indentation",
            "-o", LIB, srcs[0]]
+    if SANITIZE:
+        cmd[1:2] = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
     subprocess.run(cmd, check=True)
     return LIB
 

@@ -7,7 +7,8 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MOLSIM_LIB") or os.path.join(HERE, "libmolsim.so")   # override: tuning builds
+# MOLSIM_CHECKS=1 (tests only) loads the checked build, libmolsim_checked.so (build.py; device-side bound checks)
+LIB_PATH = os.path.join(HERE, "libmolsim_checked.so" if os.environ.get("MOLSIM_CHECKS") == "1" else "libmolsim.so")
 N_KERNELS = 10
 E_INVAL, E_CAPACITY, E_IDSPACE, E_CUDA = -1, -2, -3, -4
 

@@ -3,7 +3,9 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB = os.path.join(HERE, "libmolsim.so")
+# MOLSIM_CHECKS=1: the checked build (device-side bound checks on every data-derived index, csrc/device_types.cuh)
+CHECKED = os.environ.get("MOLSIM_CHECKS") == "1"
+LIB = os.path.join(HERE, "libmolsim_checked.so" if CHECKED else "libmolsim.so")
 SRC = os.path.join(HERE, "csrc", "molsim.cu")
 DEPS = [SRC, os.path.join(HERE, "csrc", "kernels.cuh"), os.path.join(HERE, "csrc", "device_types.cuh"),
         os.path.join(HERE, "csrc", "readout.cuh"),
@@ -16,6 +18,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
            "-shared", "-Xcompiler", "-fPIC", "-o", LIB, SRC]
+    if CHECKED:
+        cmd.insert(1, "-DMOLSIM_CHECKS=1")
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.run(cmd, check=True)

@@ -103,6 +103,16 @@ struct Params {
   unsigned long long chan_mask;    // bit s: species s has unimolecular channels
 };
 
+// Checked build (-DMOLSIM_CHECKS, paper_2606_14603_b200/build.py MOLSIM_CHECKS=1 -> libmolsim_checked.so): every index the
+// kernels derive from data (cell keys, destination slots, queue positions, look-up ranges) is tested against its
+// bound and a violation sets err bit 3 (SIM_E_INTERNAL).  compute-sanitizer is closed on this GPU pool; the GPU parity
+// tests run once against this build instead (profiles/r2_sanitizers.md).  The normal build compiles the checks away.
+#ifdef MOLSIM_CHECKS
+#define MOLSIM_CHECK(p, cond) do { if (!(cond)) atomicOr(&(p).scal->err, 8u); } while (0)
+#else
+#define MOLSIM_CHECK(p, cond) do { } while (0)
+#endif
+
 __device__ __forceinline__ bool fire(uint32_t u, uint32_t thr) { return thr == 0xFFFFFFFFu || u < thr; }
 
 // Mirror about -1/2 and L - 1/2 (S5), branch-free: -1 - q == ~q, and for 0 <= a < 2L the reflected

@@ -297,6 +297,7 @@ __global__ void __launch_bounds__(kMoveThreads, kMinBlk) k_scatter(Params p) {
     for (int a = 0; a < kK3Unroll; ++a) {
       const uint32_t dst = __shfl_sync(0xFFFFFFFFu, first[a], leader[a]) + rank[a];
       if (s[a] == kDead) continue;
+      MOLSIM_CHECK(p, key[a] < p.n_cells && dst < p.capacity);
       p.oth.r[dst] = make_int4(x[a], y[a], z[a], (int32_t)id[a]);     // ONE scattered 128-bit store per agent
       p.oth.sp[dst] = s[a];
     }
@@ -409,6 +410,7 @@ __device__ __forceinline__ void prefetch_l1(const void* ptr) { asm volatile("pre
 __device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t j, uint32_t id, uint32_t idj, uint32_t d2,
                                            uint32_t si) {
   const DevTables* __restrict__ T = p.tab;
+  MOLSIM_CHECK(p, i < p.capacity && j < p.capacity && si < (uint32_t)kMaxSpecies && p.oth.sp[j] < (uint32_t)kMaxSpecies);
   const uint32_t e = T->rxmap[si * kMaxSpecies + p.oth.sp[j]];
   if (e == 0xFFu) return;
   const DevRx& rx = T->rx[e];
@@ -449,6 +451,7 @@ __device__ __forceinline__ void scan_rows(const Params& p, PairSmem& S, uint32_t
   // groups of four records in flight, branch-free (one predicate bit each), one branch per group.  A group
   // may run up to three slots past j1: those are later slots of the sorted array (a genuine forward pair if
   // they pass) or past the population (never queued: j < n); the record array has slack for them
+  MOLSIM_CHECK(p, j1 <= n && (j0 >= j1 || j1 + 3u < p.capacity + (uint32_t)(kPairThreads + kPairHalo)));
   for (uint32_t j = j0; j < j1; j += 4u) {
     uint32_t hits = 0;
 #pragma unroll
@@ -530,14 +533,17 @@ __device__ __noinline__ uint32_t pair_drain(const Params* pp, PairSmem* Sp, uint
     if (c == 4u) { j0 = ge.x + 1u + (uint32_t)kPairWin; j1 = p.cell[ge.y + xp + 1u]; }       // own-row remainder
     else {
       const uint32_t c0 = ge.y + (uint32_t)p.fwd_row[c - 5u];      // host-precomputed row offsets of codes 5..8
+      MOLSIM_CHECK(p, c0 >= xm && c0 + xp + 1u <= p.n_cells);
       j0 = p.cell[c0 - xm]; j1 = p.cell[c0 + xp + 1u];
     }
+    MOLSIM_CHECK(p, ge.y + xp + 1u <= p.n_cells && e0 + lane < 64u);
     scan_rows(p, S, warp, j0, j1, n, ge.x, (uint32_t)o.w, ge.z >> 16, o.x, o.y, o.z);
   }
   __syncwarp();            // every lane has read its entry: the slots may be overwritten
   const uint32_t again = __ballot_sync(0xFFFFFFFFu, left != 0u);
   if (left) {
     const uint32_t k = e0 + (uint32_t)__popc(again & ((1u << lane) - 1u));
+    MOLSIM_CHECK(p, k < 64u);
     ge.z = (ge.z & ~0x1F0u) | left;
     S.ent_pos[warp][k] = o; S.ent_geo[warp][k] = ge;
     prefetch_l1(first_lookup(p, ge.y, left, ge.z >> 9 & 1u, ge.z >> 10 & 1u));
@@ -639,6 +645,7 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
     const uint32_t any = __ballot_sync(0xFFFFFFFFu, rows != 0u);
     if (rows) {
       const uint32_t k = nent + (uint32_t)__popc(any & ((1u << lane) - 1u));
+      MOLSIM_CHECK(p, k < 64u && cell < p.n_cells);
       S.ent_pos[warp][k] = q;
       S.ent_geo[warp][k] = make_uint4(i, cell, rows | (s << 16), 0u);
       prefetch_l1(first_lookup(p, cell, rows & 0x1F0u, rows >> 9 & 1u, rows >> 10 & 1u));
@@ -693,6 +700,7 @@ __global__ void __launch_bounds__(256) k_resolve(const __grid_constant__ Params 
       const uint32_t idj = (uint32_t)p.best[i];            // low word of (d2, id of the proposed partner)
       uint32_t j = p.prop[i];
       if (j >= n || (uint32_t)p.oth.r[j].w != idj) j = find_partner(&p, i, idj);
+      MOLSIM_CHECK(p, j < n);                                 // the partner named by the key exists
       if (j <= i || j >= n) continue;                         // the lower slot handles the pair
       const uint32_t idi = (uint32_t)p.oth.r[i].w;
       if ((uint32_t)p.best[j] != idi) continue;               // not mutual (best[j] = kNoKey if j never proposed)
@@ -772,6 +780,7 @@ __device__ __forceinline__ void uni_one(const Params& p, const DevTables* __rest
     atomicAdd(&p.birth_mid[id >> kMidShift], (uint32_t)__popc(mask));     // newborn counts per 256 ids and per
     atomicAdd(&p.birth_top[id >> p.top_shift], (uint32_t)__popc(mask));   // 2^top_shift ids: K6 ranks from these
     const uint32_t e = atomicAdd(&p.scal->birth_count, 1u);
+    MOLSIM_CHECK(p, e < p.capacity && id < p.id_capacity);
     p.birth_list[e] = make_uint2(i, mask | ((uint32_t)s0 << 16));
   }
 }
@@ -874,6 +883,7 @@ __global__ void __launch_bounds__(kUniThreads, kMinBlk) k_uni_hist(Params p) {
       for (uint32_t a = 0; a < 4u; ++a) {
         int leader; uint32_t rank, count;
         run_of_key(key[a], lane, leader, rank, count);
+        MOLSIM_CHECK(p, s[a] == kDead || key[a] < p.n_cells);
         if (s[a] != kDead && rank == 0u) atomicAdd(&hist[key[a]], count);     // result unused: a reduction, no round trip
       }
     }
@@ -953,6 +963,7 @@ __global__ void __launch_bounds__(kScanThreads) k_births(Params p) {
           if (c.shape == 0) { qx = mirror(qx, c.L); qy = mirror(qy, c.L); qz = mirror(qz, c.L); }
           else if (!comp_valid(c, qx, qy, qz)) { qx = lx; qy = py; qz = pz; }
           const uint32_t dst = n_sorted + rank;
+          MOLSIM_CHECK(p, dst < p.capacity && rank < total);
           p.oth.r[dst] = make_int4(qx + rbase, qy, qz, (int32_t)(next_id + rank));
           p.oth.sp[dst] = sp_new;
           // the newborn's cell in the next step's sort

@@ -272,6 +272,7 @@ int read_scalars(sim* s, Scalars* out) {
 }
 
 int err_from_bits(uint32_t bits) {
+  if (bits & 8u) return SIM_E_INTERNAL;
   if (bits & 4u) return SIM_E_INVAL;
   if (bits & 1u) return SIM_E_CAPACITY;
   if (bits & 2u) return SIM_E_IDSPACE;
@@ -828,6 +829,7 @@ const char* sim_strerror(int code) {
     case SIM_E_CAPACITY: return "capacity exceeded (agent slots, counts rows or output buffer)";
     case SIM_E_IDSPACE: return "id space exhausted";
     case SIM_E_CUDA: return "CUDA error";
+    case SIM_E_INTERNAL: return "internal bound check failed (checked build)";
     default: return "unknown error";
   }
 }
