@@ -33,7 +33,7 @@ CASES = {
     "w2_full": (lambda: configs.w2(n_steps=20), 20, "[CFG 2] full size, 8 replicas (dose sweep, PAPER.md:80-82)"),
     "w3_full": (lambda: configs.w3(**W3_TRACE), None,
                 "[CFG 3] full size, with a 50 nm gene locus, 2,000 nuclear pERK seeded at t = 0 and the repressor delay "
-                "shortened to 200 steps so that transcription, export, translation and the delayed rule all happen "
+                "shortened to 200 steps so that gene binding, transcription and the delayed rule all happen "
                 "inside the trace (cFos expression, PAPER.md:153-167; workloads/configs.py w3)"),
 }
 W3_TRACE = dict(n_steps=800, delay=200, gene_radius=500, primed_perk_n=2000)

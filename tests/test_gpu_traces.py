@@ -75,8 +75,13 @@ def test_full_size_runs_follow_the_oracle_trace(gpu, case, make):
 
 
 def test_w3_full_size_expression_follows_the_oracle_trace(gpu):
-    """[CFG 3] at full size through first transcription, mRNA export, translation and the delayed repressor."""
-    from tests.golden.make_traces import W3_TRACE
+    """[CFG 3] at full size through gene binding, first transcription and the delayed repressor."""
+    import importlib.util
+
+    spec = importlib.util.spec_from_file_location("make_traces", os.path.join(GOLDEN, "make_traces.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    W3_TRACE = mod.W3_TRACE
 
     rows = read_trace("w3_full")
     m = configs.w3(**W3_TRACE)
@@ -85,7 +90,7 @@ def test_w3_full_size_expression_follows_the_oracle_trace(gpu):
     c = np.stack([r[5] for r in rows])
     t_first = rows[-1][4]
     assert t_first != 0xFFFFFFFF and t_first + W3_TRACE["delay"] < len(rows) - 1      # the trace covers the delayed rule
-    assert c[:, ix["mRNA_n"]].max() > 0 and c[:, ix["mRNA_c"]].max() > 0              # transcription and export
+    assert c[:, ix["mRNA_n"]].max() > 0 and c[:, ix["GENE:pERK"]].max() > 0           # gene bound, transcription
     born = t_first + W3_TRACE["delay"] + 1                                            # row after the step that emits F_n
     assert c[born - 1, ix["F_n"]] + c[born - 1, ix["GENE:F"]] == 0
     assert c[born, ix["F_n"]] + c[born, ix["GENE:F"]] == 2                            # one repressor per gene locus
