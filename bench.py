@@ -109,6 +109,29 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": smax, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def kernel_source_hash():
+    """sha256 over the CUDA sources: profiles/traffic.json is stamped with it, so ncu-derived constants (DRAM traffic,
+    warp instructions per agent) are only quoted for the kernels they were measured on."""
+    import hashlib
+
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2606_14603_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -147,66 +170,57 @@ def moved_bytes_per_agent(kernel, c):
 
 
 # ------------------------------------------------------------------------------------------------
-def run_reference(args):
-    """The oracle as it stands on the host cores: each step a bounded sample of the workload."""
+def oracle_sample_model(args, steps_total):
+    """The ONE bounded sample both oracle legs time: the bench workload's recipe at a size the single-threaded oracle
+    gets through in tens of seconds ([CFG 4]: same density, N <= --oracle-n; the sphere workloads: --scale 0.1)."""
+    sargs = argparse.Namespace(**vars(args))
+    if args.workload == "w4":
+        sargs.n = min(args.n, args.oracle_n)
+    elif args.scale is None:
+        sargs.scale = 0.1
+    return make_model(sargs, steps_total)
+
+
+def time_oracle(args, warmup, steps):
     from oracle.binding import Oracle
 
+    m = oracle_sample_model(args, warmup + steps + 2)
+    o = Oracle(m)
+    o.seed_population()
+    o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    c = o.read_counts()
+    agent_steps = float(c[warmup:warmup + steps].sum())
+    full = make_model(args, 4)
+    sample = (f"{steps} step(s) after {warmup} untimed, same recipe and density at N0={m.n_agents0} "
+              f"(bench workload N0={full.n_agents0}); {dt:.1f} s of CPU work; oracle grid back end, 1 thread, g++ -O2")
+    return {"value": agent_steps / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+            "host_cpus": os.cpu_count(), "cpu_model": cpu_model()}, dt, m
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores, on the bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_sample = min(args.n, args.ref_n) if args.workload == "w4" else None
-    sargs = argparse.Namespace(**vars(args))
-    if args.workload == "w4":
-        sargs.n = n_sample
-    elif args.scale is None:
-        sargs.scale = 0.1
-    m = make_model(sargs, args.steps + args.warmup)
-    o = Oracle(m)
-    o.seed_population()
-    o.step(args.warmup)
-    t0 = time.perf_counter()
-    o.step(args.steps)
-    dt = time.perf_counter() - t0
-    c = o.read_counts()
-    w, k = args.warmup, args.steps
-    agent_steps = float(c[w:w + k].sum())
-    val = agent_steps / dt
-    full = make_model(args, 4)
-    sample = (f"same recipe and density at N={m.n_agents0} agents per step (full workload N={full.n_agents0}); "
-              f"{k} steps timed after {w} warm-up steps; oracle grid back end, g++ -O2")
+    cb, dt, m = time_oracle(args, args.warmup, args.steps)
     line = {
-        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": k, "warmup": w, "ms_per_step": dt * 1e3 / k, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-        "config": {"workload": workload_name(args, full)},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
-        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {"workload": workload_name(argparse.Namespace(**{**vars(args), "n": m.n_agents0}), m) +
+                               f" (bounded sample of the bench workload; what ran: N0={m.n_agents0})"},
+        "cpu_baseline": cb,
+        "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line), flush=True)
 
 
 def cpu_baseline(args):
-    """Oracle timed on this box's host cores on a bounded sample of the bench workload."""
-    from oracle.binding import Oracle
-
-    sargs = argparse.Namespace(**vars(args))
-    if args.workload == "w4":
-        sargs.n = min(args.n, args.cpu_n)
-    elif args.scale is None:
-        sargs.scale = 0.1
-    m = make_model(sargs, 8)
-    o = Oracle(m)
-    o.seed_population()
-    steps = max(1, args.cpu_steps)
-    t0 = time.perf_counter()
-    o.step(steps)
-    dt = time.perf_counter() - t0
-    c = o.read_counts()
-    agent_steps = float(c[:steps].sum())
-    return {"value": agent_steps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"{steps} step(s) of the same recipe at N={m.n_agents0} (seeding untimed), "
-                      f"{dt:.1f} s of CPU work, single thread, g++ -O2",
-            "host_cpus": os.cpu_count()}
+    """Oracle timed on this box's host cores on the same bounded sample --impl reference uses."""
+    return time_oracle(args, 1, max(1, args.cpu_steps))[0]
 
 
 def reduce_ranks(times, work, device):
@@ -274,6 +288,68 @@ def run_seeds(args):
                       "single_seed_value": one, "speedup_vs_single_seed": work / (ms_all * 1e-3) / one}), flush=True)
 
 
+def n_cells_of(m):
+    n = 1
+    for a in range(3):
+        n *= (m.extent[a] + m.cell_size - 1) // m.cell_size
+    return n
+
+
+def step_fractions(step_kernels_names, n_cells, n_live_mean, ms_per_step, peak):
+    c = n_cells / n_live_mean
+    ledger = sum(ledger_bytes_per_agent(k, c) for k in step_kernels_names) * n_live_mean
+    moved = sum(moved_bytes_per_agent(k, c) for k in step_kernels_names) * n_live_mean
+    gbs = ledger / (ms_per_step * 1e-3) / 1e9
+    return {"bytes_per_agent_step_ledger": round(ledger / n_live_mean, 1),
+            "bytes_per_agent_step_moved": round(moved / n_live_mean, 1),
+            "ledger_gbs": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_8TBs_nominal": gbs / 8000.0,
+            "moved_gbs": moved / (ms_per_step * 1e-3) / 1e9, "moved_frac_of_measured_peak": moved / (ms_per_step * 1e-3) / 1e9 / peak}
+
+
+STEP_KERNELS = ["memset_cells", "k_cell_reduce", "k_cell_scan", "k_scatter", "k_pairs", "k_resolve", "k_uni_hist", "k_births"]
+
+
+def run_sweep(args, pkg, torch, local, peak):
+    """Short device-timed runs of the rest of the metric's range (BASELINE.json: "at 1M-64M agents", five workloads) so
+    that the driver's record, not prose, holds them: a few steps each, CUDA events, clocks sampled per run."""
+    out = []
+    cases = [("w0", {}), ("w1", {}), ("w2", {}), ("w3", {}), ("w4", {"n": 1_000_000}), ("w4", {"n": 4_000_000}),
+             ("w4", {"n": 64_000_000})]
+    for wl, kw in cases:
+        if wl == args.workload and kw.get("n", args.n) == args.n:
+            continue
+        a2 = argparse.Namespace(**{**vars(args), "workload": wl, "n": kw.get("n", args.n), "scale": None, "cell_size": 0})
+        W, K = 5, (200 if wl in ("w0", "w3") else 20)
+        m = make_model(a2, W + K + 4)
+        sim = pkg.Sim(m, device=f"cuda:{local}")
+        sim.seed_population()
+        sim.step(W)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(local)
+        sampler.start()
+        torch.cuda.synchronize()
+        t0 = time.time()
+        ev0.record()
+        sim.step_async(K)
+        ev1.record()
+        torch.cuda.synchronize()
+        t1 = time.time()
+        clocks = sampler.stop(t0, t1)
+        ms = ev0.elapsed_time(ev1)
+        sim.step(0)
+        agent_steps = float(sim.read_counts(W, K).astype(np.int64).sum())
+        fr = step_fractions(STEP_KERNELS, n_cells_of(m), agent_steps / K, ms / K, peak)
+        out.append({"workload": workload_name(a2, m), "steps": K, "ms_per_step": ms / K,
+                    "value": agent_steps / (ms * 1e-3), "n_live_mean": agent_steps / K,
+                    "ledger_frac_of_measured_peak": round(fr["frac_of_measured_peak"], 4),
+                    "ledger_frac_of_8TBs_nominal": round(fr["frac_of_8TBs_nominal"], 4),
+                    "moved_gbs": round(fr["moved_gbs"], 1), "clocks": clocks})
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+    return out
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -293,81 +369,19 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    W, K = max(3, args.warmup), args.steps
+    W, K, R, SETTLE = max(3, args.warmup), args.steps, max(1, args.repeats), 3
     e2e_steps = min(K, args.e2e_steps)
-    m = make_model(args, W + K + 8 + 2 * (e2e_steps + 3))
+    m = make_model(args, W + SETTLE + K + args.prof_steps + 8)
     m.seed = m.seed + rank              # replicas only: independent populations
     m.place_seed = m.place_seed + rank
     sim = pkg.Sim(m, device=f"cuda:{local}")
     sim.seed_population()
-    n_cells = 1
-    for a in range(3):
-        n_cells *= (m.extent[a] + m.cell_size - 1) // m.cell_size
-
-    # ---- device-resident throughput: K steps between CUDA events on the sim's stream
-    sim.step(W)
-    launches0 = sim.launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local)
-    sampler.start()
-    time.sleep(0.25)
-    barrier()
-    t_wall0 = time.time()
-    ev0.record()
-    sim.step_async(K)
-    ev1.record()
-    barrier()
-    t_wall1 = time.time()
-    clocks = sampler.stop(t_wall0, t_wall1)
-    ms = ev0.elapsed_time(ev1)
-    launches = sim.launch_count() - launches0
-    sim.step(0)                                           # surfaces device errors
-    counts = sim.read_counts(W, K + 1).astype(np.int64)
-    agent_steps = float(counts[:K].sum())                 # sum_t n_live(t) over the timed steps
-    n_live_mean = agent_steps / K
-
-    # ---- per-kernel device time (events around every launch) for the roofline of the dominant kernel
-    sim.profile_enable(True)
-    sim.step(args.prof_steps)
-    kt = sim.kernel_times()
-    sim.profile_enable(False)
-    step_kernels = {k: v for k, v in kt.items() if k != "other" and v[1] > 0}
-    tot_ms = sum(v[0] for v in step_kernels.values())
-    dom = max(step_kernels, key=lambda k: step_kernels[k][0])
-    dom_ms = step_kernels[dom][0] / step_kernels[dom][1]
-    c_per_agent = n_cells / n_live_mean
+    n_cells = n_cells_of(m)
     peak, peak_src = measured_peak()
-    n_live_prof = float(sim.read_counts(W + K, args.prof_steps).sum()) / args.prof_steps
-    dom_bytes = ledger_bytes_per_agent(dom, n_cells / n_live_prof) * n_live_prof
-    achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
-    traffic, alu = None, None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        try:
-            tj = json.load(open(tpath))
-            traffic = tj.get(f"{args.workload}:{args.n}", {}).get(dom)
-            ipa = tj.get("warp_instr_per_agent", {}).get(f"{args.workload}:{args.n}", {}).get(dom)
-            if ipa:
-                # issue roofline of the dominant kernel: warp-instructions per launch (ncu count per
-                # agent x live agents) / launch time, against SMs x 4 schedulers x 1 instruction per clock x SM clock
-                peak_ginstr = 148 * 4 * 1.965
-                ach = ipa * n_live_prof / (dom_ms * 1e-3) / 1e9
-                alu = {"bound": "alu", "achieved": ach, "peak": peak_ginstr, "unit": "G warp-instr/s",
-                       "frac": ach / peak_ginstr, "warp_instr_per_agent": ipa,
-                       "peak_source": "148 SMs x 4 warp schedulers x 1 instr/clk x 1.965 GHz (B200_PROFILING.md clocks)"}
-        except Exception:
-            traffic, alu = None, None
-    step_bytes = sum(ledger_bytes_per_agent(k, c_per_agent) for k in step_kernels) * n_live_mean
-    moved_bytes = sum(moved_bytes_per_agent(k, c_per_agent) for k in step_kernels) * n_live_mean
-    per_kernel = {k: {"ms": round(v[0] / v[1], 4), "share": round(v[0] / tot_ms, 4),
-                      "ledger_gbs": round(ledger_bytes_per_agent(k, n_cells / n_live_prof) * n_live_prof /
-                                          (v[0] / v[1] * 1e-3) / 1e9, 1),
-                      "moved_gbs": round(moved_bytes_per_agent(k, n_cells / n_live_prof) * n_live_prof /
-                                         (v[0] / v[1] * 1e-3) / 1e9, 1)}
-                  for k, v in step_kernels.items()}
 
-    # ---- end to end through the C ABI with HOST buffers: H2D of the state, one step, D2H of the counts row
+    # ---- the state every repeat starts from: W warm-up steps, then read back into pinned host memory
     import ctypes as C
+    sim.step(W)
     state = sim.read_agents()
     n_host = len(state["id"])
     pinned = {k: torch.from_numpy(v.view(np.int32) if v.dtype == np.uint32 else
@@ -375,37 +389,127 @@ def run_gpu(args):
               for k, v in state.items()}
     info = sim.info()
     lib = pkg.load_library()
-    row = np.zeros((1, m.n_replicas, len(m.species)), dtype=np.uint32)
 
-    def e2e_step(step_no):
+    def reload_state():
         r = lib.sim_load_agents(sim._h, n_host, C.c_void_p(pinned["x"].data_ptr()), C.c_void_p(pinned["y"].data_ptr()),
                                 C.c_void_p(pinned["z"].data_ptr()), C.c_void_p(pinned["species"].data_ptr()),
-                                C.c_void_p(pinned["id"].data_ptr()), step_no, info["next_id"])
+                                C.c_void_p(pinned["id"].data_ptr()), info["step"], info["next_id"])
         assert r == 0, r
+
+    # ---- device-resident throughput: R repeats, each from the same reloaded state: SETTLE untimed steps (the reload
+    # hands the agents over in id order; the first sort puts them back in cell order), then K steps between CUDA events
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    t_wall0 = time.time()
+    rep_ms, rep_work, launches = [], [], 0
+    for r in range(R):
+        reload_state()
+        sim.step(SETTLE)
+        launches0 = sim.launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record()
+        sim.step_async(K)
+        ev1.record()
+        barrier()
+        rep_ms.append(ev0.elapsed_time(ev1))
+        launches = sim.launch_count() - launches0
+        sim.step(0)                                           # surfaces device errors
+        counts = sim.read_counts(W + SETTLE, K + 1).astype(np.int64)
+        rep_work.append(float(counts[:K].sum()))              # sum_t n_live(t) over the timed steps
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1)
+
+    # ---- per-kernel device time (events around every launch) for the roofline of the dominant kernel
+    sim.profile_enable(True)
+    sim.step(args.prof_steps)
+    kt = sim.kernel_times()
+    sim.profile_enable(False)
+    step_kernels = {k: v for k, v in kt.items() if k not in ("other", "k_hist_prologue") and v[1] > 0}
+    tot_ms = sum(v[0] for v in step_kernels.values())
+    dom = max(step_kernels, key=lambda k: step_kernels[k][0])
+    dom_ms = step_kernels[dom][0] / step_kernels[dom][1]
+    n_live_prof = float(sim.read_counts(W + SETTLE + K, args.prof_steps).sum()) / args.prof_steps
+    c_prof = n_cells / n_live_prof
+    per_kernel = {k: {"ms": round(v[0] / v[1], 4), "share": round(v[0] / tot_ms, 4),
+                      "ledger_gbs": round(ledger_bytes_per_agent(k, c_prof) * n_live_prof / (v[0] / v[1] * 1e-3) / 1e9, 1),
+                      "moved_gbs": round(moved_bytes_per_agent(k, c_prof) * n_live_prof / (v[0] / v[1] * 1e-3) / 1e9, 1)}
+                  for k, v in step_kernels.items()}
+
+    # ncu-derived constants of the dominant kernel (DRAM bytes and warp instructions per launch), quoted only while the
+    # CUDA sources are the ones they were measured on (profiles/traffic.json carries their hash)
+    traffic, ipa, traffic_src = None, None, None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    src_hash = kernel_source_hash()
+    if os.path.exists(tpath):
+        try:
+            tj = json.load(open(tpath))
+            if tj.get("source_sha16") == src_hash:
+                ent = tj.get(f"{args.workload}:{args.n}", {}).get(dom)
+                if ent:
+                    traffic, ipa, traffic_src = ent.get("dram_bytes"), ent.get("warp_instr_per_agent"), tj.get("profile")
+        except Exception:
+            pass
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the state, one step, D2H of the counts row
+    row = np.zeros((1, m.n_replicas, len(m.species)), dtype=np.uint32)
+
+    def e2e_step():
+        reload_state()
         assert lib.sim_step(sim._h, 1) == 0
-        assert lib.sim_read_counts(sim._h, step_no + 1, 1, row.ctypes.data_as(C.c_void_p)) == 0
+        assert lib.sim_read_counts(sim._h, info["step"] + 1, 1, row.ctypes.data_as(C.c_void_p)) == 0
         return int(row.sum())
 
-    base_step = info["step"]
     for i in range(2):
-        e2e_step(base_step)
+        e2e_step()
     barrier()
     t0 = time.perf_counter()
     for i in range(e2e_steps):
-        e2e_step(base_step)
+        e2e_step()
     barrier()
     e2e_dt = time.perf_counter() - t0
     e2e_agent_steps = float(n_host) * e2e_steps
 
-    # ---- reduce over ranks: max time, summed work
+    # ---- reduce over ranks: max time per repeat, summed work
     if world > 1:
-        (ms, e2e_dt), (agent_steps, e2e_agent_steps, launches) = reduce_ranks(
-            [ms, e2e_dt], [agent_steps, e2e_agent_steps, float(launches)], dev)
+        tt, ww = reduce_ranks(rep_ms + [e2e_dt], rep_work + [e2e_agent_steps, float(launches)], dev)
+        rep_ms, e2e_dt = tt[:R], tt[R]
+        rep_work, e2e_agent_steps, launches = ww[:R], ww[R], ww[R + 1]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    value = agent_steps / (ms * 1e-3)
+    rates = [w / (t * 1e-3) for w, t in zip(rep_work, rep_ms)]
+    med = int(np.argsort(rates)[len(rates) // 2])          # the median repeat
+    ms, agent_steps, value = rep_ms[med], rep_work[med], rates[med]
+    n_live_mean = agent_steps / K / world
+    fr = step_fractions(list(step_kernels), n_cells, n_live_mean, ms / K, peak)
+
+    # roofline of the dominant kernel.  k_pairs is bound by integer instruction issue, not by HBM:
+    # with ncu's instruction count of the same sources it is reported against the issue peak, else by its ledger bytes
+    if ipa:
+        peak_ginstr = 148 * 4 * 1.965
+        ach = ipa * n_live_prof / (dom_ms * 1e-3) / 1e9
+        roof = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": peak_ginstr, "unit": "G warp-instr/s",
+                "frac": ach / peak_ginstr, "traffic": traffic,
+                "peak_source": "148 SMs x 4 warp schedulers x 1 instr/clk x 1.965 GHz (B200_PROFILING.md clocks; DESIGN.md §6)",
+                "warp_instr_per_agent": ipa, "ncu_profile": traffic_src}
+    else:
+        dom_bytes = ledger_bytes_per_agent(dom, c_prof) * n_live_prof
+        ach = dom_bytes / (dom_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": None, "peak_source": peak_src,
+                "note": "no ncu constants for these sources (profiles/traffic.json hash differs): ledger bytes / event time"}
+    roof.update({"kernel_ms": dom_ms, "kernel_share_of_step": step_kernels[dom][0] / tot_ms,
+                 "hbm_ledger_gbs": round(ledger_bytes_per_agent(dom, c_prof) * n_live_prof / (dom_ms * 1e-3) / 1e9, 1),
+                 "whole_step": {"achieved": fr["ledger_gbs"], "frac": fr["frac_of_measured_peak"],
+                                "frac_of_8TBs_nominal": fr["frac_of_8TBs_nominal"], "moved_gbs": fr["moved_gbs"],
+                                "moved_frac": fr["moved_frac_of_measured_peak"], "peak": peak, "peak_source": peak_src,
+                                "what": "ledger = SURVEY 8(d) Design B bytes / device time (the contract's number); moved = the "
+                                        "bytes this implementation has to move (DESIGN.md §6): the honest companion"},
+                 "per_kernel": per_kernel,
+                 "per_kernel_note": "k_uni_hist's ledger charges K1 + K5 of the survey (48 B + 8c per agent); it moves 18 B + 8c"})
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -414,23 +518,25 @@ def run_gpu(args):
                    "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)",
                    "l2": "inputs larger than L2 (agent-store ping-pong %.0f MB vs 126 MB L2), no flush" %
                          (2 * BYTES_PER_AGENT * n_live_mean / 1e6),
-                   "bytes_per_agent_step_ledger": round(step_bytes / n_live_mean, 1),
-                   "bytes_per_agent_step_moved": round(moved_bytes / n_live_mean, 1)},
+                   "bytes_per_agent_step_ledger": fr["bytes_per_agent_step_ledger"],
+                   "bytes_per_agent_step_moved": fr["bytes_per_agent_step_moved"],
+                   "kernel_source_sha16": src_hash},
+        "repeats": {"n": R, "what": f"each repeat: sim_load_agents of the same state (step {info['step']}), {SETTLE} untimed steps, "
+                                    f"{K} timed steps; value = median repeat",
+                    "ms_per_step": [round(t / K, 5) for t in rep_ms], "spread": (max(rates) - min(rates)) / value},
         "clocks": clocks,
         "e2e": {"value": e2e_agent_steps / e2e_dt, "unit": UNIT,
                 "h2d_bytes_per_step": BYTES_PER_AGENT * n_host, "d2h_bytes_per_step": int(row.nbytes),
                 "steps": e2e_steps,
                 "what": "sim_load_agents(pinned host SoA) + sim_step(1) + sim_read_counts(1 row) per step"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                     "kernel_ms": dom_ms, "kernel_share_of_step": step_kernels[dom][0] / tot_ms, "alu": alu,
-                     "whole_step": {"achieved": step_bytes / (ms / K * 1e-3) / 1e9,
-                                    "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
-                                    "frac_of_8TBs_nominal": step_bytes / (ms / K * 1e-3) / 1e9 / 8000.0,
-                                    "moved_gbs": moved_bytes / (ms / K * 1e-3) / 1e9},
-                     "per_kernel": per_kernel},
+        "roofline": roof,
     }
+    if world == 1 and not args.no_sweep:
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+        line["sweep"] = run_sweep(args, pkg, torch, local, peak)
     if world == 1 and not args.no_cpu:
         line["cpu_baseline"] = cpu_baseline(args)
     print(json.dumps(line), flush=True)
@@ -450,9 +556,10 @@ def main():
     ap.add_argument("--cell-size", type=int, default=0)
     ap.add_argument("--prof-steps", type=int, default=5)
     ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--cpu-n", type=int, default=4_000_000, help="oracle sample size for cpu_baseline")
-    ap.add_argument("--cpu-steps", type=int, default=1)
-    ap.add_argument("--ref-n", type=int, default=1_000_000, help="oracle sample size for --impl reference")
+    ap.add_argument("--oracle-n", type=int, default=1_000_000, help="agents of the bounded sample both oracle legs time (w4)")
+    ap.add_argument("--cpu-steps", type=int, default=5, help="timed oracle steps of the cpu_baseline leg")
+    ap.add_argument("--repeats", type=int, default=5, help="timed repeats from the same reloaded state (median reported)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the short runs of the other workloads / sizes")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--seeds", type=int, default=1, help="N1: concurrent independent populations on one GPU (not the contract line)")
     args = ap.parse_args()

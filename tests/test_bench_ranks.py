@@ -58,9 +58,10 @@ def test_reference_arm_rank1_exits_without_work():
 def test_reference_arm_rank0_prints_contract_line():
     env = dict(os.environ, RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
-                        "--warmup", "1", "--ref-n", "20000"], capture_output=True, text=True, env=env, timeout=300)
+                        "--warmup", "1", "--oracle-n", "20000"], capture_output=True, text=True, env=env, timeout=300)
     assert r.returncode == 0, r.stderr
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["metric"] == "molecule_agent_steps_per_sec"
     assert line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
+    assert "N=20000" in line["config"]["workload"] and line["cpu_baseline"]["cpu_model"]   # names what actually ran
