@@ -84,7 +84,9 @@ typedef struct {
   uint32_t cell_size;      /* spatial-hash cell edge in units, >= max interaction radius; tuning only */
   uint64_t seed;           /* Philox key of the simulation streams (reading S2) */
   uint32_t capacity;       /* agent slots (live + dead + newborn of one step) */
-  uint32_t id_capacity;    /* ids ever issued must stay below this */
+  uint32_t id_capacity;    /* ids ever issued must stay below this.  Ids are never reused (reading S14): every RELEASE,
+                              BIRTH and DELAYED_BIRTH takes a fresh one, so a run needs about n0 + expected events; the
+                              id-indexed birth bitmap costs 0.5 B of workspace per id.  SIM_E_IDSPACE when exhausted. */
   uint32_t counts_rows;    /* rows of the per-step counts log; row t = state after t steps */
   uint32_t pad;
   const sim_species_t*     species;       /* [n_species] */
@@ -122,7 +124,9 @@ const char* sim_check_config(const sim_config_t* cfg);
 /* Bytes of DEVICE workspace sim_create needs for this configuration (0 if cfg is invalid). */
 size_t sim_workspace_bytes(const sim_config_t* cfg);
 
-/* Validates the tables (SIM_E_INVAL), copies them to the device, carves the workspace.
+/* One handle = one population in one cell volume (the paper's model: species classes, reactions, localisation,
+ * PAPER.md:45-54; the tables are the integer form of that model file, DESIGN.md §1 "State", readings S3, S4).
+ * Validates the tables (SIM_E_INVAL, rules V1-V7 above), copies them to the device, carves the workspace.
  * d_workspace: DEVICE memory, >= sim_workspace_bytes(cfg), 256-byte aligned, owned by the caller.
  * cuda_stream: a cudaStream_t (0 = default stream). */
 int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_bytes,
@@ -143,11 +147,15 @@ int sim_step(sim_t*, uint32_t n_steps);
 /* Same, but returns after enqueueing; errors surface at the next synchronising call. */
 int sim_step_async(sim_t*, uint32_t n_steps);
 
-/* Per-step species counts, rows first_row .. first_row+n_rows-1 (row <= steps done):
+/* Per-step species counts (DESIGN.md §1 phase 6, reading S22: row 0 = after seeding, row t+1 = after step t; the
+ * paper's concentration time series, is counts / (N_A V)), kept on the device while the run goes
+ * on; rows first_row .. first_row+n_rows-1 (row <= steps done):
  * out[n_rows][n_replicas][n_species], HOST. */
 int sim_read_counts(sim_t*, uint32_t first_row, uint32_t n_rows, uint32_t* out);
 
-/* Live agents sorted by id into HOST arrays of `cap` elements each (any array may be NULL);
+/* The agent store (north_star (1): int32 x, y, z in 0.1 nm units, uint16 species, uint32 id; DESIGN.md §1 "State")
+ * read back; it stands in for the paper's 3-D view of the molecules.  Memory order on the device is
+ * unspecified (reading S23), so the live agents are returned sorted by id into HOST arrays of `cap` elements each (any array may be NULL);
  * *n_out = number of live agents (also set when cap is too small: SIM_E_CAPACITY). */
 int sim_read_agents(sim_t*, uint32_t cap, int32_t* x, int32_t* y, int32_t* z,
                     uint16_t* species, uint32_t* id, uint32_t* n_out);
@@ -194,6 +202,8 @@ int sim_profile_enable(sim_t*, int on);
 int sim_kernel_times(sim_t*, float ms[SIM_N_KERNELS], uint32_t launches[SIM_N_KERNELS]);
 const char* sim_kernel_name(int k);
 
+/* Waits for the stream, releases the handle's graphs, streams and host state (north_star boundary list).  The
+ * workspace stays the caller's. */
 void sim_destroy(sim_t*);
 const char* sim_strerror(int code);
 const char* sim_last_cuda_error(const sim_t*);

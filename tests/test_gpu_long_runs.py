@@ -94,9 +94,12 @@ def test_w2_full_size_dose_sweep(gpu):
 
 
 def test_w3_full_size_expression(gpu):
-    """[CFG 3] in full for 6,000 steps: compartment invariant for every agent, mRNA and cFos appear, the
-    delayed repressor is born exactly `delay` steps after the first transcription."""
-    m = configs.w3(n_steps=6000)
+    """[CFG 3] at full size for 6,000 steps (with the 50 nm gene locus and primed nuclear pERK of the trace recipe, so
+    that transcription starts: workloads/configs.py w3): compartment invariant for every agent, mRNA appears, exported
+    and translated, and the delayed repressor is born exactly `delay` = 2,000 steps after the first transcription,
+    one per gene locus.  Nothing here is conditional."""
+    delay = 2000
+    m = configs.w3(n_steps=6000, delay=delay, gene_radius=500, primed_perk_n=2000)
     sim = gpu.Sim(m); sim.seed_population(); sim.step(6000)
     c = sim.read_counts()[:, 0, :].astype(np.int64)
     ix = {s.name: i for i, s in enumerate(m.species)}
@@ -111,8 +114,11 @@ def test_w3_full_size_expression(gpu):
             assert (r2 > cmp.r_in ** 2).all()
     assert (c[:, ix["GENE"]] + c[:, ix["GENE:pERK"]] + c[:, ix["GENE:F"]] == 2).all()      # the two fixed loci
     t_first = sim.info()["t_first0"]
-    if t_first != 0xFFFFFFFF:
-        assert c[:, ix["mRNA_n"]].max() + c[:, ix["mRNA_c"]].max() > 0
+    assert t_first != 0xFFFFFFFF and t_first + delay + 1 < 6000, t_first
+    assert c[:t_first + 1, ix["mRNA_n"]].max() == 0 and c[t_first + 1, ix["mRNA_n"]] >= 1   # first transcription at t_first
+    assert c[:, ix["mRNA_c"]].max() > 0 and c[:, ix["cFos_c"]].max() > 0                    # export and translation
+    rep = c[:, ix["F_n"]] + c[:, ix["GENE:F"]]
+    assert (rep[:t_first + delay + 1] == 0).all() and (rep[t_first + delay + 1:] == 2).all()  # born at t_first + delay
 
 
 @pytest.mark.parametrize("n", [1_000_000, 4_000_000, 16_000_000, pytest.param(64_000_000, marks=pytest.mark.slow)])

@@ -146,6 +146,29 @@ def test_compiled_physical_model_parity(gpu):
     assert np.array_equal(sim.read_counts(), orc.read_counts())
 
 
+def test_compiled_compartmentalised_model_parity(gpu):
+    """N2 with the paper's localisation / translocation / expressor / degradation fields: a
+    [CFG 3]-shaped model written in physical units, compiled, and stepped on both sides: bit-exact state and counts,
+    membrane crossings, expression and degradation included."""
+    from oracle.binding import Oracle
+    from test_model_compiler import nuclear_spec
+    from workloads import compiler
+
+    m = compiler.compile_model(nuclear_spec(n_steps=400), cell_size=512)
+    sim, orc = gpu.Sim(m), Oracle(m)
+    for s in (sim, orc):
+        s.seed_population()
+    for chunk in range(4):
+        sim.step(100); orc.step(100)
+        a, b = sim.read_agents(), orc.read_agents()
+        for k in ("id", "species", "x", "y", "z"):
+            assert np.array_equal(a[k], b[k]), (chunk, k)
+    c = orc.read_counts()
+    assert np.array_equal(sim.read_counts(), c) and sim.read_checksum() == orc.read_checksum()
+    ix = {s.name: i for i, s in enumerate(m.species)}
+    assert c[:, 0, ix["mRNA_n"]].max() > 0 and c[:, 0, ix["pS"]].max() > 0        # expression and the cascade happened
+
+
 def test_derived_concentration_curves_and_perk_fraction(gpu):
     """SURVEY 8(a) a11 / [NS]: the only floating-point outputs are derived on the host in double from the integer
     counts — concentration curves c(t) = n(t) / (N_A V) and [CFG 2]'s steady-state pERK fraction (reading S19) — and
@@ -158,10 +181,15 @@ def test_derived_concentration_curves_and_perk_fraction(gpu):
     for s in (sim, orc):
         s.seed_population(); s.step(120)
     cg, co = sim.read_counts(), orc.read_counts()
-    curves_g = wm.concentration_molar(cg, m.volume_um3)
-    curves_o = wm.concentration_molar(co, m.volume_um3)
+    curves_g = wm.concentration_molar(cg, m.volume_um3)          # the product-side derivation, on the CUDA path's counts
     assert curves_g.dtype == np.float64 and curves_g.shape == cg.shape
+    # expected curve: the definition c = n / (N_A V) written out here (CODATA N_A; volume of the 5 um sphere scaled by
+    # the model's count scale, in litres), applied to the ORACLE's counts -- not the function under test
+    R_um = m.compartments[0].r_out / 10_000.0
+    litres = 4.0 / 3.0 * np.pi * R_um ** 3 * 1e-15
+    curves_o = co.astype(np.float64) / (6.02214076e23 * litres)
     nz = curves_o != 0
+    assert nz.any()
     assert np.all(np.abs(curves_g[nz] - curves_o[nz]) <= 1e-6 * np.abs(curves_o[nz])) and np.all(curves_g[~nz] == 0)
     names = [s.name for s in m.species]
     perk, erk_like = names.index("pERK"), [names.index(n) for n in ("ERK", "pERK", "pMEK:ERK", "P:pERK")]

@@ -82,3 +82,104 @@ def test_compiled_model_runs_on_the_oracle_and_conserves_moieties():
     c = o.read_counts()[:, 0, :].astype(np.int64)
     assert (c[:, 0] + c[:, 2] == c[0, 0]).all() and (c[:, 1] + c[:, 2] == c[0, 1]).all()
     assert c[-1, 2] > 0                                            # bindings happened
+
+
+# --------------------------------------------------------------------------- localisation, translocation, expressors
+def nuclear_spec(**over):
+    """A [CFG 3]-shaped model in physical units: kinase K phosphorylates S in the cytosol,
+    pS shuttles through the nuclear membrane, binds the gene locus, the bound locus expresses mRNA, which is
+    exported, translated by an expressor reaction and degraded."""
+    spec = {
+        "name": "nuclear_physical", "dt_us": 10.0, "seed": 21, "n_steps": 40,
+        "cell": {"radius_um": 0.6, "nucleus_radius_um": 0.3},
+        "molecules": [
+            {"name": "K", "mw_da": 85_000, "concentration_molar": 2.0e-6,
+             "interactions": [{"partner": "S", "complex": "K:S", "radius_nm": 5.0, "p_bind": 0.8}]},
+            {"name": "S", "mw_da": 42_000, "concentration_molar": 8.0e-6,
+             "interactions": [{"partner": "K", "complex": "K:S", "radius_nm": 5.0, "p_bind": 0.8}]},
+            {"name": "K:S", "mw_da": 127_000, "release": {"kcat_per_s": 5_000.0, "products": ["K", "pS"]}},
+            {"name": "pS", "mw_da": 42_000, "translocation": {"to": "pS_n", "prob_per_contact": 0.05}},
+            {"name": "pS_n", "mw_da": 42_000, "localisation": "nucleus", "concentration_molar": 3.0e-6,
+             "translocation": {"to": "pS", "prob_per_contact": 0.05},
+             "interactions": [{"partner": "GENE", "complex": "GENE:pS", "radius_nm": 40.0, "p_bind": 0.5}]},
+            {"name": "GENE", "mw_da": 1_000_000, "localisation": "nucleus", "immobile": True, "count": 2,
+             "interactions": [{"partner": "pS_n", "complex": "GENE:pS", "radius_nm": 40.0, "p_bind": 0.5}]},
+            {"name": "GENE:pS", "mw_da": 1_042_000, "localisation": "nucleus", "immobile": True,
+             "expression": {"product": "mRNA_n", "rate_per_s": 20_000.0},
+             "release": {"kcat_per_s": 200.0, "products": ["GENE", "pS_n"]}},
+            {"name": "mRNA_n", "mw_da": 400_000, "localisation": "nucleus", "degradation_per_s": 5.0,
+             "translocation": {"to": "mRNA_c", "prob_per_contact": 0.02}},
+            {"name": "mRNA_c", "mw_da": 400_000, "degradation_per_s": 5.0,
+             "expression": {"product": "P", "rate_per_s": 100.0}},
+            {"name": "P", "mw_da": 40_000, "degradation_per_s": 2.0},
+        ],
+    }
+    spec.update(over)
+    return spec
+
+
+def test_compartmentalised_model_compiles_to_shell_nucleus_twins_and_channels():
+    spec = nuclear_spec()
+    assert compiler.check(spec) == []
+    m = compiler.compile_model(spec, cell_size=512)
+    R, Rn = 6000, 3000
+    shell, nuc = m.compartments
+    assert (shell.shape, shell.r_out, shell.r_in, nuc.r_out, nuc.r_in) == (model.SHAPE_SPHERE, R, Rn, Rn, -1)
+    assert m.extent == (2 * R + 1,) * 3
+    ix = {s.name: i for i, s in enumerate(m.species)}
+    assert [m.species[ix[n]].compartment for n in ("K", "pS", "pS_n", "GENE", "mRNA_n", "mRNA_c")] == [0, 0, 1, 1, 1, 0]
+    # counts: concentration x volume of the molecule's OWN compartment (closed form, PAPER.md:84-97)
+    v_cyt = 4.0 / 3.0 * math.pi * (0.6 ** 3 - 0.3 ** 3) * 1e-15
+    v_nuc = 4.0 / 3.0 * math.pi * 0.3 ** 3 * 1e-15
+    want = {"K": round(2.0e-6 * model.N_AVOGADRO * v_cyt), "S": round(8.0e-6 * model.N_AVOGADRO * v_cyt),
+            "pS_n": round(3.0e-6 * model.N_AVOGADRO * v_nuc), "GENE": 2}
+    got = {m.species[r.species].name: r.count for r in m.seed_records}
+    assert got == want and want["pS_n"] == 204
+    # translocation -> twin species and the per-contact threshold, both directions; mRNA export is one-way
+    assert (m.species[ix["pS"]].cross_to, m.species[ix["pS_n"]].cross_to) == (ix["pS_n"], ix["pS"])
+    assert m.species[ix["pS"]].cross_thr == model.prob_to_thr(0.05) == 214748365
+    assert m.species[ix["mRNA_n"]].cross_to == ix["mRNA_c"] and m.species[ix["mRNA_c"]].cross_to == model.NONE16
+    # expressor -> BIRTH with 1 - exp(-rate dt), before the consuming channels; degradation -> DEGRADE last
+    g = m.species[ix["GENE:pS"]].channels
+    assert [c.kind for c in g] == [model.CH_BIRTH, model.CH_RELEASE]
+    assert g[0].prod1 == ix["mRNA_n"] and g[0].thr == model.prob_to_thr(1 - math.exp(-20_000.0 * 10e-6))
+    assert (g[1].prod0, g[1].prod1) == (ix["GENE"], ix["pS_n"])
+    r = m.species[ix["mRNA_c"]].channels
+    assert [c.kind for c in r] == [model.CH_BIRTH, model.CH_DEGRADE] and r[1].thr == model.prob_to_thr(1 - math.exp(-5.0 * 10e-6))
+    assert m.species[ix["GENE"]].sigma_class == 0 and m.species[ix["GENE:pS"]].sigma_class == 0        # immobile loci
+    assert m.species[ix["pS"]].sigma_class == m.species[ix["S"]].sigma_class != 0
+    import paper_2606_14603_b200 as pkg
+    assert pkg.check_config(m) is None                                  # the compiled tables pass the library's checker
+
+
+def test_checker_reports_compartment_mismatches():
+    s = nuclear_spec(); s["molecules"][4]["interactions"][0]["partner"] = "K"          # nuclear pS_n binding cytosolic K
+    assert any("partner K is localised in the cytosol, not the nucleus" in f for f in compiler.check(s))
+    s = nuclear_spec(); s["molecules"][3]["translocation"]["to"] = "S"                  # twin in the same compartment
+    assert any("translocation target S is localised in the same compartment" in f for f in compiler.check(s))
+    s = nuclear_spec(); s["molecules"][8]["expression"]["product"] = "mRNA_n"           # cytosolic expressor, nuclear product
+    assert any("expressed product mRNA_n is localised in the nucleus, not the cytosol" in f for f in compiler.check(s))
+    s = nuclear_spec(); s["molecules"][6]["release"]["products"] = ["GENE", "pS"]       # nuclear complex releasing into the cytosol
+    assert any("release product pS is localised in the cytosol, not the nucleus" in f for f in compiler.check(s))
+    s = nuclear_spec(); del s["cell"]; s["volume_l"] = 1e-15                            # nucleus without a cell geometry
+    assert any("needs a cell geometry with a nucleus" in f for f in compiler.check(s))
+    s = nuclear_spec(); s["cell"]["nucleus_radius_um"] = 0.7
+    assert any("nucleus_radius_um < radius_um" in f for f in compiler.check(s))
+    s = nuclear_spec(); s["molecules"][3]["translocation"]["to"] = "nowhere"
+    assert any("unknown molecule 'nowhere'" in f for f in compiler.check(s))
+
+
+def test_compartmentalised_model_runs_on_the_oracle():
+    from oracle.binding import Oracle
+
+    m = compiler.compile_model(nuclear_spec(n_steps=300), cell_size=512)
+    o = Oracle(m); o.seed_population(); o.step(300)
+    a = o.read_agents()
+    c = o.read_counts()[:, 0, :].astype(np.int64)
+    ix = {s.name: i for i, s in enumerate(m.species)}
+    comp = np.array([s.compartment for s in m.species])[a["species"]]
+    r2 = sum((a[k].astype(np.int64) - 6000) ** 2 for k in "xyz")
+    assert ((r2[comp == 0] > 3000 ** 2) & (r2[comp == 0] <= 6000 ** 2)).all() and (r2[comp == 1] <= 3000 ** 2).all()
+    assert (c[:, ix["GENE"]] + c[:, ix["GENE:pS"]] == 2).all()                            # the two loci
+    assert (c[:, ix["K"]] + c[:, ix["K:S"]] == c[0, ix["K"]]).all()                       # kinase moiety
+    assert c[:, ix["pS"]].max() > 0 and c[:, ix["GENE:pS"]].max() > 0 and c[:, ix["mRNA_n"]].max() > 0
