@@ -504,14 +504,8 @@ __device__ __forceinline__ PairGeo pair_geo(const Params& p, int32_t x, int32_t 
   return g;
 }
 
-// Address of the first cell-range word the row with the lowest code in `rows` will look up.
-__device__ __forceinline__ const uint32_t* first_lookup(const Params& p, uint32_t cell, uint32_t rows, uint32_t xm, uint32_t xp) {
-  const uint32_t c = (uint32_t)__ffs(rows) - 1u;
-  return p.cell + (c == 4u ? cell + xp + 1u : cell + (uint32_t)p.fwd_row[c - 5u] - xm);
-}
-
 // C / D for one warp.  Takes up to 32 entries off the top of its queue and visits ONE row of each (two cell-range
-// look-ups, whose line was prefetched when the entry was queued, then records in groups of four); an entry with
+// look-ups, then records in groups of four); an entry with
 // further rows goes back on the queue, so every round is dense and costs one memory round trip.  Then, if there are
 // enough of them (or `all`), the warp's hits.  Returns the new queue length.  Out of line: its registers (Philox,
 // 64-bit keys) must not be charged to the dense per-tile loop.
@@ -546,7 +540,6 @@ __device__ __noinline__ uint32_t pair_drain(const Params* pp, PairSmem* Sp, uint
     MOLSIM_CHECK(p, k < 64u);
     ge.z = (ge.z & ~0x1F0u) | left;
     S.ent_pos[warp][k] = o; S.ent_geo[warp][k] = ge;
-    prefetch_l1(first_lookup(p, ge.y, left, ge.z >> 9 & 1u, ge.z >> 10 & 1u));
   }
   nent = e0 + (uint32_t)__popc(again);
   __syncwarp();
@@ -640,15 +633,13 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
       if (xk <= (g.xp ? p.pack_span2 : p.pack_span1)) rows |= 1u << 4;
       if (rows) rows |= (g.xm << 9) | (g.xp << 10);
     }
-    // ---- B: one entry per agent with rows to visit, appended to the warp's queue; the cell-range words its first row
-    // will look up are asked for now
+    // ---- B: one entry per agent with rows to visit, appended to the warp's queue
     const uint32_t any = __ballot_sync(0xFFFFFFFFu, rows != 0u);
     if (rows) {
       const uint32_t k = nent + (uint32_t)__popc(any & ((1u << lane) - 1u));
       MOLSIM_CHECK(p, k < 64u && cell < p.n_cells);
       S.ent_pos[warp][k] = q;
       S.ent_geo[warp][k] = make_uint4(i, cell, rows | (s << 16), 0u);
-      prefetch_l1(first_lookup(p, cell, rows & 0x1F0u, rows >> 9 & 1u, rows >> 10 & 1u));
     }
     nent += (uint32_t)__popc(any);
     // this warp is done with the stage
