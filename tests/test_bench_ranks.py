@@ -65,3 +65,34 @@ def test_reference_arm_rank0_prints_contract_line():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
     assert "N=20000" in line["config"]["workload"] and line["cpu_baseline"]["cpu_model"]   # names what actually ran
+
+
+def test_ncu_constants_are_quoted_only_for_the_sources_they_were_measured_on():
+    """profiles/traffic.json carries a sha256 of paper_2606_14603_b200/csrc; bench.py recomputes it and drops the
+    ncu-derived fields (roofline.traffic, warp instructions per agent) when the sources have changed since."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    assert len(tj["source_sha16"]) == 16 and tj["profile"].startswith("profiles/")
+    ent = tj["w4:16000000"]["k_pairs"]
+    assert ent["dram_bytes"] > 0 and 5.0 < ent["warp_instr_per_agent"] < 15.0
+    # the committed capture belongs to the committed kernels (a kernel change must come with a new capture, or the
+    # bench line falls back to ledger bytes and says so)
+    assert bench.kernel_source_hash() == tj["source_sha16"]
+
+
+def test_ledger_and_moved_bytes_per_agent_step():
+    """SURVEY.md 8(d) Design B: 106.5 + 32c bytes per agent-step over the step's kernels; what the implementation moves
+    is smaller."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    c = 0.25
+    ledger = sum(bench.ledger_bytes_per_agent(k, c) for k in bench.STEP_KERNELS)
+    assert abs(ledger - (106.5 + 32 * c)) < 1e-9
+    moved = sum(bench.moved_bytes_per_agent(k, c) for k in bench.STEP_KERNELS)
+    assert abs(moved - (18 + 8 * c + 4 * c + 4 * c + 8 * c + 36 + 8 * c + 18.125 + 4 * c + 0.125)) < 1e-9 and moved < ledger
+    fr = bench.step_fractions(bench.STEP_KERNELS, 1_000_000, 4_000_000.0, 1.0, 6532.2)
+    assert abs(fr["ledger_gbs"] - (106.5 + 8) * 4e6 / 1e-3 / 1e9) < 1e-6
+    assert abs(fr["frac_of_8TBs_nominal"] - fr["ledger_gbs"] / 8000.0) < 1e-12
