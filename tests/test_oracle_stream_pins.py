@@ -337,3 +337,104 @@ def test_homodimer_anchor_is_the_smaller_id(torch_philox):
     alive = dict(zip(b3["id"].tolist(), b3["species"].tolist()))
     for i, j in mutual:
         assert alive.get(i) == 2 and j not in alive
+
+
+# --------------------------------------------------------------------------- replicas: local coordinates (S16)
+def test_replica_move_uses_local_coordinates_and_keeps_the_tile(torch_philox):
+    R, shift, n_rep = 1500, 12, 4
+    c = 1600
+    m = Model(name="rep", species=[Species("a", 1, 0)], reactions=[], table_bits=12, tables=stack_tables([60.0], 12),
+              compartments=[Compartment(SHAPE_SPHERE, c, c, c, r_out=R, r_in=-1)], extent=(n_rep << shift, 2 * c + 1, 2 * c + 1),
+              n_replicas=n_rep, stride_shift=shift, seed=0xD1CE, place_seed=1, seed_records=[], n_steps=16, cell_size=128).finalize()
+    o = Oracle(m)
+    rng = np.random.default_rng(3)
+    n = 2000
+    v = rng.normal(size=(n, 3)); v /= np.linalg.norm(v, axis=1)[:, None]
+    q = np.rint(c + v * (R - rng.integers(0, 60, size=n))[:, None]).astype(np.int64)          # near the surface
+    q = q[((q - c) ** 2).sum(axis=1) <= R * R]
+    n = len(q)
+    rep = rng.integers(0, n_rep, size=n)
+    ids = rng.permutation(n).astype(np.uint32)
+    o.load_agents(q[:, 0] + (rep << shift), q[:, 1], q[:, 2], np.zeros(n, np.uint16), ids, step=7, next_id=n)
+    o.debug_move_only()
+    a = o.read_agents()
+    order = np.argsort(ids)
+    q, rep, ids = q[order], rep[order], ids[order]
+    r = torch_philox(ctr(ids, 0, 7, TAG_MOVE), key_of(m.seed))
+    tab = m.tables[1].astype(np.int64)
+    qq = q + np.stack([tab[r[:, ax] >> 20] for ax in range(3)], axis=1)                     # in LOCAL coordinates
+    ok = ((qq - c) ** 2).sum(axis=1) <= R * R
+    assert ok.sum() > 300 and (~ok).sum() > 300
+    want = np.where(ok[:, None], qq, q)
+    assert (a["x"] == want[:, 0] + (rep << shift)).all() and (a["y"] == want[:, 1]).all() and (a["z"] == want[:, 2]).all()
+    assert ((a["x"] >> shift) == rep).all()                                                  # nobody changes replica
+    cnt = o.read_counts()[-1, :, 0]
+    assert (cnt == np.bincount(rep, minlength=n_rep)).all()                                  # counts are per replica
+
+
+# --------------------------------------------------------------------------- delayed births (S17) and expressors
+def test_delayed_birth_fires_exactly_delay_steps_after_the_first_marked_birth(torch_philox):
+    from workloads.model import CH_DELAYED_BIRTH
+
+    L, delay, p0 = 400, 4, 0.04
+    G, Mx, F = 0, 1, 2
+    thr = prob_to_thr(p0)
+    m = Model(name="delay", species=[
+        Species("G", 0, channels=[Channel(CH_BIRTH, thr, prod1=Mx, rule=0, marks_first=True),
+                                  Channel(CH_DELAYED_BIRTH, delay, prod1=F, rule=0)]),
+        Species("M", 0), Species("F", 0)], reactions=[], compartments=[Compartment(SHAPE_CUBE, L=L)], table_bits=12,
+        tables=stack_tables([10.0], 12), extent=(L, L, L), seed=0xC0DE00, place_seed=4, n_rules=1,
+        seed_records=[SeedRecord(G, 6)], n_steps=40, cell_size=64).finalize()
+    o = Oracle(m); o.seed_population()
+    g = o.read_agents()
+    gid = g["id"]
+    gpos = np.stack([g["x"], g["y"], g["z"]], axis=1).astype(np.int64)
+    key = key_of(m.seed)
+    T = 30
+    rows, t_first, next_id = [], None, 6
+    born_ids, born_sp, born_pos = [], [], []
+    for t in range(T):
+        u = torch_philox(ctr(gid, 0, t, TAG_UNI), key)
+        fired0 = fire(u[:, 0], thr)                                    # channel 0 reads word r0
+        delayed = t_first is not None and t == t_first + delay          # t_first as of the start of the step
+        for k_parent in range(6):                                       # (parent id, channel) order: ids ascend with k_parent
+            for ch, on, spc in ((0, fired0[k_parent], Mx), (1, delayed, F)):
+                if not on:
+                    continue
+                b = torch_philox(ctr([gid[k_parent]], ch, t, TAG_BIRTH), key).astype(np.uint64)[0]
+                off = ((b[:3] * 21) >> 32).astype(np.int64) - 10
+                born_ids.append(next_id); next_id += 1
+                born_sp.append(spc); born_pos.append(mirror(gpos[k_parent] + off, L))
+        if fired0.any() and t_first is None:
+            t_first = t
+        rows.append((6, born_sp.count(Mx), born_sp.count(F)))
+    assert t_first is not None and t_first + delay < T - 2 and t_first > 0
+    o.step(T)
+    a, c = o.read_agents(), o.read_counts()[:, 0, :]
+    assert o.info()["t_first0"] == t_first and o.info()["next_id"] == next_id
+    assert (c[1:] == np.array(rows)).all()
+    assert c[t_first + delay, F] == 0 and c[t_first + delay + 1, F] == 6      # every locus emits one, exactly then, once
+    assert (a["id"][6:] == np.array(born_ids)).all() and (a["species"][6:] == np.array(born_sp)).all()
+    bp = np.array(born_pos)
+    for ax, k in enumerate("xyz"):
+        assert (a[k][6:] == bp[:, ax]).all(), k
+
+
+# --------------------------------------------------------------------------- mid-run seeding (run-time treatment)
+def test_mid_run_seeding_continues_ids_and_uses_its_own_place_seed(torch_philox):
+    m = ab_model(L=900, n_a=100, n_b=0, p_bind=0.5, seed=11)
+    o = Oracle(m); o.seed_population()
+    o.step(2)
+    before, n0 = o.read_agents(), o.info()["next_id"]
+    o.seed_population([SeedRecord(1, 50), SeedRecord(0, 7)], place_seed=0xFEED)
+    a = o.read_agents()
+    new = a["id"] >= n0
+    assert new.sum() == 57 and (a["id"][new] == n0 + np.arange(57)).all()
+    assert (a["species"][new] == np.repeat([1, 0], [50, 7])).all()
+    r = torch_philox(ctr(a["id"][new], 0, 0, TAG_PLACE), key_of(0xFEED)).astype(np.uint64)
+    for ax, k in enumerate("xyz"):
+        assert (a[k][new] == ((r[:, ax] * 900) >> 32).astype(np.int32)).all(), k
+        assert (a[k][~new] == before[k]).all()                          # the old agents are untouched
+    c = o.read_counts()
+    assert c.shape[0] == 3 and list(c[2, 0]) == [int((a["species"] == s).sum()) for s in range(3)]   # row t rewritten
+    assert o.info()["step"] == 2 and o.info()["next_id"] == n0 + 57
