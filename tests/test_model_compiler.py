@@ -183,3 +183,16 @@ def test_compartmentalised_model_runs_on_the_oracle():
     assert (c[:, ix["GENE"]] + c[:, ix["GENE:pS"]] == 2).all()                            # the two loci
     assert (c[:, ix["K"]] + c[:, ix["K:S"]] == c[0, ix["K"]]).all()                       # kinase moiety
     assert c[:, ix["pS"]].max() > 0 and c[:, ix["GENE:pS"]].max() > 0 and c[:, ix["mRNA_n"]].max() > 0
+
+
+def test_shipped_example_model_files_compile_and_pass_the_library_checker():
+    import os
+
+    import paper_2606_14603_b200 as pkg
+
+    d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "workloads", "examples")
+    for name, n_species in (("toy_cube.json", 3), ("nuclear_cell.json", 10)):
+        text = open(os.path.join(d, name)).read()
+        assert compiler.check(json.loads(text)) == []
+        m = compiler.compile_model(text)
+        assert len(m.species) == n_species and m.n_agents0 > 0 and pkg.check_config(m) is None
