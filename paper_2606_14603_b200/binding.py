@@ -64,7 +64,12 @@ def load_library():
     if not os.path.exists(LIB_PATH):
         raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
                           "(nvcc, sm_100a). There is no CPU fallback.")
-    L = C.CDLL(LIB_PATH)
+    _lib = declare_signatures(C.CDLL(LIB_PATH))
+    return _lib
+
+
+def declare_signatures(L):
+    """ctypes argument / result types of every export of include/molsim.h on a loaded library."""
     vp, u32, u64, P = C.c_void_p, C.c_uint32, C.c_uint64, C.POINTER
     L.sim_workspace_bytes.argtypes = [P(_Config)]
     L.sim_workspace_bytes.restype = C.c_size_t
@@ -97,7 +102,6 @@ def load_library():
     L.sim_debug_philox.argtypes = [vp, vp, vp, u32, vp]
     L.sim_monitor_eval.argtypes = [vp, vp, u32, vp, vp, u32]
     L.sim_render.argtypes = [vp, vp, vp]
-    _lib = L
     return L
 
 

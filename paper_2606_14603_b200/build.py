@@ -8,7 +8,7 @@ CHECKED = os.environ.get("MOLSIM_CHECKS") == "1"
 LIB = os.path.join(HERE, "libmolsim_checked.so" if CHECKED else "libmolsim.so")
 SRC = os.path.join(HERE, "csrc", "molsim.cu")
 DEPS = [SRC, os.path.join(HERE, "csrc", "kernels.cuh"), os.path.join(HERE, "csrc", "device_types.cuh"),
-        os.path.join(HERE, "csrc", "readout.cuh"),
+        os.path.join(HERE, "csrc", "readout.cuh"), os.path.join(HERE, "csrc", "ptx_sm100.cuh"),
         os.path.join(os.path.dirname(HERE), "include", "molsim.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 

@@ -7,6 +7,7 @@
 // histogram atomics produce inside a cell cannot change any result.
 #pragma once
 #include "device_types.cuh"
+#include "ptx_sm100.cuh"
 
 namespace molsim {
 
@@ -370,27 +371,7 @@ constexpr int kPairHitCap = 16, kPairHitDrain = 8;     // per warp
 constexpr uint32_t kPairTileBytes = (kPairThreads + kPairHalo) * 16u + kPairThreads * 2u;
 constexpr unsigned long long kNoKey = ~0ull;
 
-// ---- mbarrier + bulk copy (PTX, sm_90+; SASS on sm_100a: SYNCS / UBLKCP)
-__device__ __forceinline__ uint32_t smem_addr(const void* ptr) { return (uint32_t)__cvta_generic_to_shared(ptr); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-               : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
-  return ok != 0u;
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
-}
+// mbarrier + bulk copy + fences: ptx_sm100.cuh (PTX, sm_90+; SASS on sm_100a: SYNCS / UBLKCP)
 
 struct PairSmem {
   int4 rec[kPairStages][kPairThreads + kPairHalo];   // x, y, z, id of the tile's slots and the kPairHalo behind them
@@ -403,8 +384,6 @@ struct PairSmem {
   unsigned long long full[kPairStages], empty[kPairStages];
   uint32_t nhit[kPairWarps];
 };
-
-__device__ __forceinline__ void prefetch_l1(const void* ptr) { asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr)); }
 
 // Reaction look-up, exact radius and symmetric pair draw for the geometric hit (i, j); on success both ends are merged.
 __device__ __forceinline__ void pair_merge(const Params& p, uint32_t i, uint32_t j, uint32_t id, uint32_t idj, uint32_t d2,
@@ -559,7 +538,7 @@ __device__ __noinline__ uint32_t pair_drain(const Params* pp, PairSmem* Sp, uint
 
 __device__ __forceinline__ void pair_issue_tile(const Params& p, PairSmem& S, uint32_t stage, uint32_t tile) {
   // generic-proxy reads of this stage (by the tile that used it before) are ordered before the async-proxy refill
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  fence_proxy_async();
   mbar_expect_tx(&S.full[stage], kPairTileBytes);
   bulk_g2s(S.rec[stage], p.oth.r + (size_t)tile * kPairThreads, (kPairThreads + kPairHalo) * 16u, &S.full[stage]);
   bulk_g2s(S.sp[stage], p.oth.sp + (size_t)tile * kPairThreads, kPairThreads * 2u, &S.full[stage]);
@@ -573,7 +552,7 @@ __global__ void __launch_bounds__(kPairBlock, 4) k_pairs(const __grid_constant__
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   if (tid == 0) {
     for (int k = 0; k < kPairStages; ++k) { mbar_init(&S.full[k], 1u); mbar_init(&S.empty[k], (uint32_t)kPairWarps); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_mbar_init();
   }
   if (lane == 0 && warp < (uint32_t)kPairWarps) S.nhit[warp] = 0;
   __syncthreads();                  // the only block-wide barrier

@@ -364,12 +364,14 @@ bool capture_steps(sim* s, uint32_t steps, cudaGraphExec_t* out) {
 void build_graphs(sim* s) {
   s->graphs_tried = true;
   if (cudaStreamCreateWithFlags(&s->cap, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return; }
+  const Params saved = s->prm;
   bool ok = true;
   for (int k = 0; k < 2 && ok; ++k) {
     const int par = parity_of(s);
     ok = capture_steps(s, 1, &s->g1[par]) && capture_steps(s, kGraphSteps, &s->g8[par]);
     flip(s);   // the other parity (flipped back by the second round)
   }
+  s->prm = saved;   // a capture that fails in the first round must not leave the ping-pong flipped for the direct launches
   s->graphs_ok = ok;
 }
 

@@ -1,0 +1,59 @@
+// ptx_sm100_emu.cuh — TEST INFRASTRUCTURE (see simt_shim.h).  Host stand-ins for the inline-PTX helpers of
+// paper_2606_14603_b200/csrc/ptx_sm100.cuh, with the semantics the PTX ISA gives them: an mbarrier has an arrival
+// count and a transaction-byte count; a phase completes when both reach zero, which flips the phase bit and re-arms the
+// arrival count; try_wait.parity(P) is true once the phase with parity P has completed.  A bulk copy moves its bytes
+// and credits them to the barrier; its operands must be 16-byte aligned and the size a multiple of 16 (checked).
+// tests/simt/build.py installs this file as "ptx_sm100.cuh" of the emulation build.
+#pragma once
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+namespace molsim {
+
+struct EmuMbar { uint32_t phase : 1, pending : 15, count : 16; int32_t tx; };
+static_assert(sizeof(EmuMbar) == 8, "an mbarrier is one 64-bit shared-memory word");
+
+inline EmuMbar* emu_bar(unsigned long long* bar) { return reinterpret_cast<EmuMbar*>(bar); }
+inline void emu_bar_settle(EmuMbar* m) {
+  if (m->pending == 0 && m->tx == 0) { m->phase ^= 1u; m->pending = m->count; }
+  simt::note_progress();
+}
+inline void emu_fail(const char* what) { std::fprintf(stderr, "simt ptx: %s\n", what); std::abort(); }
+
+inline void mbar_init(unsigned long long* bar, uint32_t count) {
+  EmuMbar* m = emu_bar(bar);
+  m->phase = 0; m->pending = count; m->count = count; m->tx = 0;
+}
+inline void fence_mbar_init() {}
+inline void mbar_expect_tx(unsigned long long* bar, uint32_t bytes) {
+  EmuMbar* m = emu_bar(bar);
+  if (m->pending == 0) emu_fail("mbarrier arrival beyond the expected count");
+  m->tx += (int32_t)bytes; m->pending--;
+  emu_bar_settle(m);
+}
+inline void mbar_arrive(unsigned long long* bar) {
+  EmuMbar* m = emu_bar(bar);
+  if (m->pending == 0) emu_fail("mbarrier arrival beyond the expected count");
+  m->pending--;
+  emu_bar_settle(m);
+}
+inline bool mbar_try_wait(unsigned long long* bar, uint32_t parity) {
+  if (emu_bar(bar)->phase != (parity & 1u)) return true;
+  simt::yield();                         // the callers spin on this
+  return false;
+}
+inline void fence_proxy_async() {}
+inline void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
+  if (((uintptr_t)dst | (uintptr_t)src | bytes) & 15u) emu_fail("bulk copy operands must be 16-byte aligned multiples of 16");
+  std::memcpy(dst, src, bytes);
+  EmuMbar* m = emu_bar(bar);
+  m->tx -= (int32_t)bytes;
+  emu_bar_settle(m);
+}
+inline void prefetch_l1(const void* ptr) {
+  (void)*reinterpret_cast<const volatile unsigned char*>(ptr);     // a prefetch of an unmapped address is dropped on the
+}                                                                  // GPU; here it must at least lie inside an allocation
+
+}  // namespace molsim

@@ -1,0 +1,44 @@
+"""TEST INFRASTRUCTURE: the cases tests/test_simt_kernels.py runs in a child process against the sanitizer build of the
+emulation (-fsanitize=address,undefined; libasan preloaded).  `python san_cases.py overrun` is the self-test that must
+die with an AddressSanitizer report."""
+import ctypes as C
+import os
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path[:0] = [os.path.dirname(os.path.dirname(HERE)), os.path.dirname(HERE), HERE]
+
+from harness import Emu, load  # noqa: E402
+
+
+def main():
+    if sys.argv[1:] == ["overrun"]:
+        L = load(sanitize=True)
+        L.simt_selftest_overrun.argtypes = [C.c_void_p, C.c_size_t]
+        p = L.simt_alloc(4096)
+        L.simt_selftest_overrun(p, 4096)
+        print("SIMT-SAN the overrun went unnoticed")
+        return
+    import test_gpu_parity as gp
+    import test_gpu_readouts as gr
+    import test_gpu_traces as gt
+
+    from workloads import configs
+
+    def w3_shell_and_nucleus(e):       # membrane crossings, no-flux walls, expression channels
+        gp.run_both(e, configs.w3(scale=0.004, n_steps=60, cell_size=1024), 60, chunks=2)
+
+    emu = Emu(sanitize=True)
+    cases = [gp.test_seeding_parity_all_geometries, gp.test_move_only_parity, gp.test_tiny_dense_cube_many_events,
+             gp.test_large_displacements, gp.test_channel_kinds_and_priority, gp.test_crowded_single_cell,
+             gp.test_empty_population_and_mid_run_seeding, gp.test_errors, gt.test_homodimer_parity,
+             gt.test_load_agents_rejects_bad_positions_and_duplicate_ids, gr.test_picture_parity_nucleus_and_cytoplasm,
+             w3_shell_and_nucleus]
+    for c in cases:
+        c(emu)
+        print("SIMT-SAN case ok:", c.__name__, flush=True)
+    print(f"SIMT-SAN OK {len(cases)} cases, {load(True).simt_launches()} kernel launches", flush=True)
+
+
+if __name__ == "__main__":
+    main()
