@@ -41,16 +41,20 @@ inline void mbar_arrive(unsigned long long* bar) {
 }
 inline bool mbar_try_wait(unsigned long long* bar, uint32_t parity) {
   if (emu_bar(bar)->phase != (parity & 1u)) return true;
+  simt::run_deferred(bar);               // adversarial mode: a copy lands no earlier than the first poll that waits for it
   simt::yield();                         // the callers spin on this
   return false;
 }
 inline void fence_proxy_async() {}
 inline void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
   if (((uintptr_t)dst | (uintptr_t)src | bytes) & 15u) emu_fail("bulk copy operands must be 16-byte aligned multiples of 16");
-  std::memcpy(dst, src, bytes);
-  EmuMbar* m = emu_bar(bar);
-  m->tx -= (int32_t)bytes;
-  emu_bar_settle(m);
+  auto land = [=]() {
+    std::memcpy(dst, src, bytes);
+    EmuMbar* m = emu_bar(bar);
+    m->tx -= (int32_t)bytes;
+    emu_bar_settle(m);
+  };
+  if (!simt::defer(bar, land)) land();
 }
 inline void prefetch_l1(const void* ptr) {
   (void)*reinterpret_cast<const volatile unsigned char*>(ptr);     // a prefetch of an unmapped address is dropped on the

@@ -22,6 +22,7 @@ def main():
     import test_gpu_parity as gp
     import test_gpu_readouts as gr
     import test_gpu_traces as gt
+    import test_zz_gpu_global_tables as gz
 
     from workloads import configs
 
@@ -29,11 +30,10 @@ def main():
         gp.run_both(e, configs.w3(scale=0.004, n_steps=60, cell_size=1024), 60, chunks=2)
 
     emu = Emu(sanitize=True)
-    cases = [gp.test_seeding_parity_all_geometries, gp.test_move_only_parity, gp.test_tiny_dense_cube_many_events,
-             gp.test_large_displacements, gp.test_channel_kinds_and_priority, gp.test_crowded_single_cell,
+    cases = [gp.test_move_only_parity, gp.test_tiny_dense_cube_many_events, gp.test_channel_kinds_and_priority, gp.test_crowded_single_cell,
              gp.test_empty_population_and_mid_run_seeding, gp.test_errors, gt.test_homodimer_parity,
              gt.test_load_agents_rejects_bad_positions_and_duplicate_ids, gr.test_picture_parity_nucleus_and_cytoplasm,
-             w3_shell_and_nucleus]
+             w3_shell_and_nucleus, gz.body_large_gaussian_tables]
     for c in cases:
         c(emu)
         print("SIMT-SAN case ok:", c.__name__, flush=True)

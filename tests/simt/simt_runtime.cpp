@@ -99,6 +99,16 @@ Block B;
 SimtGraph* g_capture = nullptr;
 unsigned long long g_switches = 0, g_launches = 0;
 
+// Adversarial mode (SIMT_SCHED_SEED != 0): blocks run in a random order, every scheduler pass visits a random subset of
+// the live fibres in a random order, and deferred work (bulk copies) lands as late as it legally can.  Whatever the
+// schedule, the results must not change: that is the race / ordering check (a missing barrier, a queue shared between
+// warps, a result that depends on which atomic wins, a stage read before its copy landed all show as a mismatch).
+unsigned long long g_rng = 0;
+bool g_adversarial = false;
+unsigned rnd() { g_rng ^= g_rng << 13; g_rng ^= g_rng >> 7; g_rng ^= g_rng << 17; return (unsigned)(g_rng >> 32); }
+struct Deferred { const void* key; std::function<void()> fn; };
+std::vector<Deferred> g_deferred;
+
 void fibre_entry() {
 #if SIMT_ASAN
   __sanitizer_finish_switch_fiber(nullptr, &B.main_bottom, &B.main_size);
@@ -135,11 +145,16 @@ void run_block(unsigned n) {
     f.done = false; f.fake = nullptr;
   }
   unsigned idle = 0;
+  static unsigned order[kMaxThreads];
+  for (unsigned t = 0; t < n; ++t) order[t] = t;
   while (B.alive) {
     const unsigned long long before = B.progress;
-    for (unsigned t = 0; t < n; ++t) {
+    if (g_adversarial) for (unsigned t = n - 1; t > 0; --t) std::swap(order[t], order[rnd() % (t + 1u)]);
+    for (unsigned k = 0; k < n; ++k) {
+      const unsigned t = order[k];
       Fibre& f = B.fib[t];
       if (f.done) continue;
+      if (g_adversarial && (rnd() & 3u) == 0u) continue;          // this fibre sits the pass out
       B.cur = t; g.tid.x = t;
       ++g_switches;
 #if SIMT_ASAN
@@ -162,10 +177,17 @@ void execute_grid(unsigned grid, unsigned block, size_t smem, const std::functio
   B.body = &body;
   B.dyn = smem ? std::malloc(smem) : nullptr;      // its own allocation: ASan sees an overrun of the dynamic shared memory
   g.bdim = uint3{block, 1, 1}; g.gdim = uint3{grid, 1, 1};
-  for (unsigned b = 0; b < grid; ++b) {
+  const char* seed = std::getenv("SIMT_SCHED_SEED");
+  g_adversarial = seed && std::atoll(seed) != 0;
+  if (g_adversarial) { g_rng = (unsigned long long)std::atoll(seed) * 0x9E3779B97F4A7C15ull + g_launches; rnd(); rnd(); }
+  std::vector<unsigned> blocks(grid);
+  for (unsigned b = 0; b < grid; ++b) blocks[b] = b;
+  if (g_adversarial) for (unsigned b = grid; b > 1; --b) std::swap(blocks[b - 1], blocks[rnd() % b]);
+  for (unsigned b : blocks) {
     g.bid = uint3{b, 0, 0};
     if (B.dyn) std::memset(B.dyn, 0xCD, smem);     // shared memory starts as garbage in every block
     run_block(block);
+    if (!g_deferred.empty()) die("a bulk copy was still in flight when its block ended");
   }
   std::free(B.dyn); B.dyn = nullptr; B.body = nullptr;
 }
@@ -183,6 +205,17 @@ void yield() {
 #endif
 }
 void note_progress() { B.progress++; }
+bool defer(const void* key, std::function<void()> fn) {
+  if (!g_adversarial) return false;                // the caller does the work now
+  g_deferred.push_back(Deferred{key, std::move(fn)});
+  return true;
+}
+void run_deferred(const void* key) {
+  for (size_t k = 0; k < g_deferred.size();) {
+    if (g_deferred[k].key == key) { auto fn = std::move(g_deferred[k].fn); g_deferred.erase(g_deferred.begin() + k); fn(); }
+    else ++k;
+  }
+}
 void* dyn_smem() { return B.dyn; }
 
 void syncthreads() {

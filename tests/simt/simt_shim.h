@@ -49,6 +49,8 @@ extern Builtins g;
 void yield();                                  // back to the block scheduler; resumed later
 void note_progress();                          // something another fibre may be waiting for has happened
 void* dyn_smem();                              // the launch's dynamic shared memory
+bool defer(const void* key, std::function<void()> fn);   // adversarial mode: queue fn under key, true; else false
+void run_deferred(const void* key);            // run (and forget) everything queued under key
 void syncthreads();
 // Warp rendezvous: every live lane named in `mask` deposits v; each gets all deposits and who took part.
 void warp_exchange(unsigned mask, unsigned long long v, unsigned long long out[32], unsigned* participants);

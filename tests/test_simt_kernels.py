@@ -30,6 +30,7 @@ sys.path[:0] = [p for p in (os.path.join(HERE, "simt"), HERE) if p not in sys.pa
 import test_gpu_parity as gp  # noqa: E402
 import test_gpu_readouts as gr  # noqa: E402
 import test_gpu_traces as gt  # noqa: E402
+import test_zz_gpu_global_tables as gz  # noqa: E402
 from workloads import configs  # noqa: E402
 
 
@@ -89,6 +90,7 @@ def test_rewrites_are_the_three_stated_ones():
     gt.test_homodimer_parity, gt.test_checksum_equals_oracle_and_sees_every_field,
     gt.test_w3_checkpoint_reload_with_t_first, gt.test_load_agents_rejects_bad_positions_and_duplicate_ids,
     gr.test_picture_parity_nucleus_and_cytoplasm, gr.test_compiled_compartmentalised_model_parity,
+    gz.body_large_gaussian_tables,
 ], ids=lambda f: f.__name__)
 def test_gpu_test_body_on_the_emulation(emu, body):
     body(emu)
@@ -162,3 +164,31 @@ def test_sanitizer_sees_an_overrun_inside_a_kernel():
     r = subprocess.run([sys.executable, os.path.join(HERE, "simt", "san_cases.py"), "overrun"], env=env,
                        capture_output=True, text=True, timeout=600)
     assert r.returncode != 0 and "heap-buffer-overflow" in r.stderr and "went unnoticed" not in r.stdout
+
+
+# ------------------------------------------------------------------------------------------------ schedules and races
+@pytest.mark.parametrize("seed", [1, 2])
+def test_results_do_not_depend_on_the_schedule(emu, monkeypatch, seed):
+    """Blocks in a random order, a random subset of the fibres in a random order on every scheduler pass, bulk copies that
+    land only when somebody waits for them: the result is still the oracle's, bit for bit (every decision is keyed by id,
+    min over 64-bit keys is order-free, and no kernel relies on who wins an atomic or on lock-step warps)."""
+    monkeypatch.setenv("SIMT_SCHED_SEED", str(seed))
+    gp.test_tiny_dense_cube_many_events(emu)
+    gp.test_channel_kinds_and_priority(emu)
+    gp.test_crowded_single_cell(emu)
+    gt.test_homodimer_parity(emu)
+    gp.run_both(emu, configs.w4(n=30_011, n_steps=17), 17, chunks=1)
+    gp.run_both(emu, configs.w3(scale=0.004, n_steps=60, cell_size=1024), 60, chunks=2)
+
+
+@pytest.mark.parametrize("name,seed", [("window_keys_without_syncwarp", 0), ("tile_read_without_full_wait", 1),
+                                       ("hit_reset_without_syncwarp", 0), ("histogram_before_species_final", 1),
+                                       ("resolve_trusts_prop", 1)])
+def test_a_removed_synchronisation_is_noticed(name, seed):
+    """The check above has teeth: with one synchronisation taken out of the emulation's copy of the kernels (mutants.py) the
+    same cases no longer match the oracle (or trip a bound check, the deadlock report, or crash)."""
+    env = dict(os.environ)
+    env.pop("SIMT_NO_GRAPHS", None)
+    r = subprocess.run([sys.executable, os.path.join(HERE, "simt", "mutants.py"), name, str(seed)], env=env,
+                       capture_output=True, text=True, timeout=900)
+    assert r.returncode != 0 and "SURVIVED" not in r.stdout, f"mutant {name} survived:\n{r.stdout[-500:]}"

@@ -1,0 +1,60 @@
+"""GPU parity for the one kernel configuration no other test reaches: Gaussian displacement tables too large for shared
+memory (> 160 KB: 16-bit tables, or many sigma classes), where K3 / K5 / the prologue / the move hook are the
+`kGaussSmem = false` instantiations that read the tables from global memory.  Found by line coverage of the emulation
+build (tests/test_simt_kernels.py), which runs the same body on the CPU; this file was added while the GPU pool was
+closed to the repository, so it is collected last: a failure here cannot hide another GPU test behind `pytest -x`."""
+import numpy as np
+import pytest
+
+from workloads.model import (CH_RELEASE, SHAPE_CUBE, SHAPE_SPHERE, Channel, Compartment, Model, Reaction, SeedRecord,
+                             Species, prob_to_thr, stack_tables)
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_14603_b200 as pkg
+
+    pkg.load_library()
+    return pkg
+
+
+def big_table_models():
+    A, B, Cx = 0, 1, 2
+    sp = [Species("A", 1), Species("B", 2), Species("C", 3, channels=[Channel(CH_RELEASE, prob_to_thr(0.03), A, B)])]
+    rx = [Reaction(A, B, Cx, 2500, prob_to_thr(0.6))]
+    # 4 rows x 2^16 entries x 2 B = 512 KB of tables
+    cube = Model(name="tables16_cube", species=sp, reactions=rx, compartments=[Compartment(SHAPE_CUBE, L=450)],
+                 table_bits=16, tables=stack_tables([44.7214, 31.6228, 20.0], 16), extent=(450,) * 3, seed=31,
+                 place_seed=32, seed_records=[SeedRecord(A, 2100), SeedRecord(B, 1900)], n_steps=30, cell_size=64).finalize()
+    # 24 sigma classes x 2^12 entries x 2 B = 196 KB, in a sphere (no-flux wall)
+    sig = [10.0 + 3.0 * k for k in range(23)]
+    sp2 = [Species("A", 23), Species("B", 7), Species("C", 1, channels=[Channel(CH_RELEASE, prob_to_thr(0.03), A, B)])]
+    R = 400
+    sphere = Model(name="tables24_sphere", species=sp2, reactions=rx,
+                   compartments=[Compartment(SHAPE_SPHERE, cx=R, cy=R, cz=R, r_out=R, r_in=-1)], table_bits=12,
+                   tables=stack_tables(sig, 12), extent=(2 * R + 1,) * 3, seed=33, place_seed=34,
+                   seed_records=[SeedRecord(A, 2500), SeedRecord(B, 2500)], n_steps=30, cell_size=100).finalize()
+    return cube, sphere
+
+
+def body_large_gaussian_tables(gpu):
+    from test_gpu_parity import oracle_cls, run_both
+
+    for m in big_table_models():
+        assert m.tables.nbytes > 160 * 1024
+        run_both(gpu, m, 30, chunks=3)
+        sim = gpu.Sim(m); orc = oracle_cls()(m)              # the move-only hook has its own instantiation
+        sim.seed_population(); orc.seed_population()
+        sim.debug_move_only(); orc.debug_move_only()
+        a, b = sim.read_agents(), orc.read_agents()
+        for k in ("id", "species", "x", "y", "z"):
+            assert (a[k] == b[k]).all(), (m.name, k)
+
+
+@pytest.mark.gpu
+def test_large_gaussian_tables_in_global_memory(gpu):
+    body_large_gaussian_tables(gpu)
