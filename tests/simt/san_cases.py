@@ -30,13 +30,22 @@ def main():
         gp.run_both(e, configs.w3(scale=0.004, n_steps=60, cell_size=1024), 60, chunks=2)
 
     emu = Emu(sanitize=True)
-    cases = [gp.test_move_only_parity, gp.test_tiny_dense_cube_many_events, gp.test_channel_kinds_and_priority, gp.test_crowded_single_cell,
-             gp.test_empty_population_and_mid_run_seeding, gp.test_errors, gt.test_homodimer_parity,
+    def random_models(e):              # 30 random models: every shape, channel kind, homodimers, replicas, crowded volumes
+        from paper_2606_14603_b200.binding import check_config
+        from random_models import fuzz_parity
+
+        assert fuzz_parity(e, range(200, 230), check_config, gp.oracle_cls(), gp.assert_same) >= 25
+
+    cases = [gp.test_tiny_dense_cube_many_events, gp.test_channel_kinds_and_priority, gp.test_crowded_single_cell,
+             gt.test_homodimer_parity, gp.test_empty_population_and_mid_run_seeding, gp.test_errors,
              gt.test_load_agents_rejects_bad_positions_and_duplicate_ids, gr.test_picture_parity_nucleus_and_cytoplasm,
-             w3_shell_and_nucleus, gz.body_large_gaussian_tables]
+             w3_shell_and_nucleus, gz.body_large_gaussian_tables, random_models]
+    import time
+
     for c in cases:
+        t0 = time.time()
         c(emu)
-        print("SIMT-SAN case ok:", c.__name__, flush=True)
+        print(f"SIMT-SAN case ok: {c.__name__} ({time.time() - t0:.1f} s)", flush=True)
     print(f"SIMT-SAN OK {len(cases)} cases, {load(True).simt_launches()} kernel launches", flush=True)
 
 

@@ -319,8 +319,9 @@ void* simt_alloc(size_t bytes) {
   void* p = nullptr;
   if (posix_memalign(&p, 256, bytes)) return nullptr;
   unsigned long long x = 0x9E3779B97F4A7C15ull;
-  unsigned char* q = (unsigned char*)p;
-  for (size_t i = 0; i < bytes; ++i) { x ^= x << 13; x ^= x >> 7; x ^= x << 17; q[i] = (unsigned char)(x >> 24); }
+  unsigned long long* q = (unsigned long long*)p;
+  for (size_t i = 0; i < bytes / 8; ++i) { x ^= x << 13; x ^= x >> 7; x ^= x << 17; q[i] = x; }
+  for (size_t i = bytes & ~(size_t)7; i < bytes; ++i) ((unsigned char*)p)[i] = 0xA5;
   return p;
 }
 void simt_free(void* p) { std::free(p); }

@@ -58,3 +58,15 @@ def body_large_gaussian_tables(gpu):
 @pytest.mark.gpu
 def test_large_gaussian_tables_in_global_memory(gpu):
     body_large_gaussian_tables(gpu)
+
+
+@pytest.mark.gpu
+def test_random_models_parity(gpu):
+    """Parity fuzzing: 60 seeded random models (tests/random_models.py: cubes, spheres, shell + nucleus with membrane twins,
+    replicas; random species, sigma classes, reactions up to R = cell size, every channel kind) stepped on the GPU and on
+    the oracle; full state, counts, info and checksum compared.  The CPU tier runs the same body on the emulation."""
+    from paper_2606_14603_b200.binding import check_config
+    from random_models import fuzz_parity
+    from test_gpu_parity import assert_same, oracle_cls
+
+    assert fuzz_parity(gpu, range(1000, 1060), check_config, oracle_cls(), assert_same) >= 50
