@@ -10,46 +10,52 @@
 #include <cstdlib>
 #include <cstring>
 
+// The barrier words themselves are touched by many fibres between rendezvous: not data, so not for ThreadSanitizer.
+#define EMU_BAR __attribute__((no_sanitize("thread")))
+
 namespace molsim {
 
 struct EmuMbar { uint32_t phase : 1, pending : 15, count : 16; int32_t tx; };
 static_assert(sizeof(EmuMbar) == 8, "an mbarrier is one 64-bit shared-memory word");
 
-inline EmuMbar* emu_bar(unsigned long long* bar) { return reinterpret_cast<EmuMbar*>(bar); }
-inline void emu_bar_settle(EmuMbar* m) {
+EMU_BAR inline EmuMbar* emu_bar(unsigned long long* bar) { return reinterpret_cast<EmuMbar*>(bar); }
+EMU_BAR inline void emu_bar_settle(EmuMbar* m) {
   if (m->pending == 0 && m->tx == 0) { m->phase ^= 1u; m->pending = m->count; }
   simt::note_progress();
 }
 inline void emu_fail(const char* what) { std::fprintf(stderr, "simt ptx: %s\n", what); std::abort(); }
 
-inline void mbar_init(unsigned long long* bar, uint32_t count) {
+EMU_BAR inline void mbar_init(unsigned long long* bar, uint32_t count) {
   EmuMbar* m = emu_bar(bar);
   m->phase = 0; m->pending = count; m->count = count; m->tx = 0;
 }
 inline void fence_mbar_init() {}
-inline void mbar_expect_tx(unsigned long long* bar, uint32_t bytes) {
+EMU_BAR inline void mbar_expect_tx(unsigned long long* bar, uint32_t bytes) {
   EmuMbar* m = emu_bar(bar);
+  simt::hb_release(bar);
   if (m->pending == 0) emu_fail("mbarrier arrival beyond the expected count");
   m->tx += (int32_t)bytes; m->pending--;
   emu_bar_settle(m);
 }
-inline void mbar_arrive(unsigned long long* bar) {
+EMU_BAR inline void mbar_arrive(unsigned long long* bar) {
   EmuMbar* m = emu_bar(bar);
+  simt::hb_release(bar);                 // what this thread did before arriving is visible to whoever waits the phase out
   if (m->pending == 0) emu_fail("mbarrier arrival beyond the expected count");
   m->pending--;
   emu_bar_settle(m);
 }
-inline bool mbar_try_wait(unsigned long long* bar, uint32_t parity) {
-  if (emu_bar(bar)->phase != (parity & 1u)) return true;
+EMU_BAR inline bool mbar_try_wait(unsigned long long* bar, uint32_t parity) {
+  if (emu_bar(bar)->phase != (parity & 1u)) { simt::hb_acquire(bar); return true; }
   simt::run_deferred(bar);               // adversarial mode: a copy lands no earlier than the first poll that waits for it
   simt::yield();                         // the callers spin on this
   return false;
 }
 inline void fence_proxy_async() {}
-inline void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
+EMU_BAR inline void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
   if (((uintptr_t)dst | (uintptr_t)src | bytes) & 15u) emu_fail("bulk copy operands must be 16-byte aligned multiples of 16");
-  auto land = [=]() {
-    std::memcpy(dst, src, bytes);
+  auto land = [=]() EMU_BAR {
+    std::memcpy(dst, src, bytes);          // the async proxy's write, done by whichever fibre lands the copy
+    simt::hb_release(bar);
     EmuMbar* m = emu_bar(bar);
     m->tx -= (int32_t)bytes;
     emu_bar_settle(m);

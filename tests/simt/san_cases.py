@@ -1,9 +1,11 @@
-"""TEST INFRASTRUCTURE: the cases tests/test_simt_kernels.py runs in a child process against the sanitizer build of the
-emulation (-fsanitize=address,undefined; libasan preloaded).  `python san_cases.py overrun` is the self-test that must
-die with an AddressSanitizer report."""
+"""TEST INFRASTRUCTURE: the cases tests/test_simt_kernels.py runs in a child process against a sanitizer build of the
+emulation: `python san_cases.py` = -fsanitize=address,undefined (libasan preloaded), `python san_cases.py tsan` =
+ThreadSanitizer on the kernels (libtsan preloaded; one TSan fibre per CUDA thread, happens-before only where CUDA gives
+it).  `python san_cases.py overrun` is the self-test that must die with an AddressSanitizer report."""
 import ctypes as C
 import os
 import sys
+import time
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 sys.path[:0] = [os.path.dirname(os.path.dirname(HERE)), os.path.dirname(HERE), HERE]
@@ -29,7 +31,8 @@ def main():
     def w3_shell_and_nucleus(e):       # membrane crossings, no-flux walls, expression channels
         gp.run_both(e, configs.w3(scale=0.004, n_steps=60, cell_size=1024), 60, chunks=2)
 
-    emu = Emu(sanitize=True)
+    mode = "tsan" if sys.argv[1:] == ["tsan"] else True
+    emu = Emu(sanitize=mode)
     def random_models(e):              # 30 random models: every shape, channel kind, homodimers, replicas, crowded volumes
         from paper_2606_14603_b200.binding import check_config
         from random_models import fuzz_parity
@@ -42,11 +45,20 @@ def main():
              w3_shell_and_nucleus, gz.body_large_gaussian_tables, random_models]
     import time
 
+    if mode == "tsan":                 # the race check proper: the kernels that share queues, tiles and counters
+        def random_models_few(e):
+            from paper_2606_14603_b200.binding import check_config
+            from random_models import fuzz_parity
+
+            assert fuzz_parity(e, range(200, 212), check_config, gp.oracle_cls(), gp.assert_same) >= 9
+
+        cases = [gp.test_tiny_dense_cube_many_events, gp.test_channel_kinds_and_priority, gp.test_crowded_single_cell,
+                 gt.test_homodimer_parity, gp.test_errors, w3_shell_and_nucleus, random_models_few]
     for c in cases:
         t0 = time.time()
         c(emu)
         print(f"SIMT-SAN case ok: {c.__name__} ({time.time() - t0:.1f} s)", flush=True)
-    print(f"SIMT-SAN OK {len(cases)} cases, {load(True).simt_launches()} kernel launches", flush=True)
+    print(f"SIMT-SAN OK {len(cases)} cases, {load(mode).simt_launches()} kernel launches", flush=True)
 
 
 if __name__ == "__main__":

@@ -59,6 +59,28 @@ extern "C" void __sanitizer_finish_switch_fiber(void* fake_stack_save, const voi
 #define SIMT_ASAN 0
 #endif
 
+// ThreadSanitizer (build mode "tsan": kernels instrumented, this file not): every CUDA thread index is a TSan fibre, switches
+// carry NO synchronisation, and the happens-before edges are exactly the ones CUDA gives: launch boundaries, __syncthreads,
+// __syncwarp, mbarrier arrive -> wait, __threadfence.  A conflicting pair of plain accesses that none of these orders is
+// reported as a data race.
+#if defined(SIMT_TSAN)
+extern "C" {
+void* __tsan_get_current_fiber(void);
+void* __tsan_create_fiber(unsigned flags);
+void __tsan_destroy_fiber(void* fiber);
+void __tsan_switch_to_fiber(void* fiber, unsigned flags);
+void __tsan_acquire(void* addr);
+void __tsan_release(void* addr);
+}
+#define TSAN_SWITCH(f) __tsan_switch_to_fiber((f), 1u /* no synchronisation */)
+#define TSAN_ACQUIRE(a) __tsan_acquire((void*)(a))
+#define TSAN_RELEASE(a) __tsan_release((void*)(a))
+#else
+#define TSAN_SWITCH(f) ((void)0)
+#define TSAN_ACQUIRE(a) ((void)0)
+#define TSAN_RELEASE(a) ((void)0)
+#endif
+
 struct SimtStream { int dummy; };
 struct SimtEvent { std::chrono::steady_clock::time_point at; };
 struct SimtGraph { std::vector<std::function<void()>> ops; };
@@ -76,10 +98,12 @@ struct Fibre {
   Context ctx;
   char* stack = nullptr;
   void* fake = nullptr;          // ASan fake-stack handle while the fibre is switched out
+  void* tsan = nullptr;          // TSan fibre of this thread index (kept across blocks and launches)
   bool done = true;
 };
 struct WarpSync {
   unsigned arrived = 0, releasing = 0, part = 0, live = 0;
+  char hb = 0;                   // happens-before token of __syncwarp
   unsigned long long val[32], snap[32];
 };
 struct Block {
@@ -94,6 +118,8 @@ struct Block {
   const std::function<void()>* body = nullptr;
   void* dyn = nullptr;
   unsigned long long progress = 0;
+  void* tsan_main = nullptr;
+  char hb_bar = 0, hb_launch_start = 0, hb_launch_end = 0, hb_fence = 0;
 };
 Block B;
 SimtGraph* g_capture = nullptr;
@@ -113,7 +139,9 @@ void fibre_entry() {
 #if SIMT_ASAN
   __sanitizer_finish_switch_fiber(nullptr, &B.main_bottom, &B.main_size);
 #endif
+  TSAN_ACQUIRE(&B.hb_launch_start);            // everything before the launch happens-before every thread of it
   (*B.body)();
+  TSAN_RELEASE(&B.hb_launch_end);
   const unsigned t = B.cur;
   B.fib[t].done = true;
   B.alive--;
@@ -122,6 +150,7 @@ void fibre_entry() {
 #if SIMT_ASAN
   __sanitizer_start_switch_fiber(nullptr, B.main_bottom, B.main_size);     // this fibre never runs again
 #endif
+  TSAN_SWITCH(B.tsan_main);
   context_switch(&B.fib[t].ctx, &B.main);
 }
 
@@ -142,6 +171,9 @@ void run_block(unsigned n) {
     Fibre& f = B.fib[t];
     if (!f.stack) f.stack = (char*)std::malloc(kStackBytes);
     context_make(&f.ctx, f.stack, kStackBytes, fibre_entry);
+#if defined(SIMT_TSAN)
+    if (!f.tsan) f.tsan = __tsan_create_fiber(0);
+#endif
     f.done = false; f.fake = nullptr;
   }
   unsigned idle = 0;
@@ -161,6 +193,7 @@ void run_block(unsigned n) {
       void* fake_main = nullptr;
       __sanitizer_start_switch_fiber(&fake_main, f.stack, kStackBytes);
 #endif
+      TSAN_SWITCH(f.tsan);
       context_switch(&B.main, &f.ctx);
 #if SIMT_ASAN
       __sanitizer_finish_switch_fiber(fake_main, nullptr, nullptr);
@@ -180,15 +213,25 @@ void execute_grid(unsigned grid, unsigned block, size_t smem, const std::functio
   const char* seed = std::getenv("SIMT_SCHED_SEED");
   g_adversarial = seed && std::atoll(seed) != 0;
   if (g_adversarial) { g_rng = (unsigned long long)std::atoll(seed) * 0x9E3779B97F4A7C15ull + g_launches; rnd(); rnd(); }
+#if defined(SIMT_TSAN)
+  B.tsan_main = __tsan_get_current_fiber();
+#endif
+  TSAN_RELEASE(&B.hb_launch_start);
   std::vector<unsigned> blocks(grid);
   for (unsigned b = 0; b < grid; ++b) blocks[b] = b;
   if (g_adversarial) for (unsigned b = grid; b > 1; --b) std::swap(blocks[b - 1], blocks[rnd() % b]);
   for (unsigned b : blocks) {
     g.bid = uint3{b, 0, 0};
     if (B.dyn) std::memset(B.dyn, 0xCD, smem);     // shared memory starts as garbage in every block
+    TSAN_RELEASE(&B.hb_launch_start);              // (again: the fill above is the host's; blocks stay unordered among themselves)
     run_block(block);
+    // Shared memory (statics, the dynamic buffer) is reused by the next block, which on the GPU has its own: for
+    // ThreadSanitizer the blocks of a launch are therefore ordered one after the other; a conflict BETWEEN blocks is
+    // what the seeded block orders of the adversarial schedules are for.
+    TSAN_ACQUIRE(&B.hb_launch_end);
     if (!g_deferred.empty()) die("a bulk copy was still in flight when its block ended");
   }
+  TSAN_ACQUIRE(&B.hb_launch_end);               // the launch happens-before whatever the host does next
   std::free(B.dyn); B.dyn = nullptr; B.body = nullptr;
 }
 
@@ -199,12 +242,16 @@ void yield() {
 #if SIMT_ASAN
   __sanitizer_start_switch_fiber(&f.fake, B.main_bottom, B.main_size);
 #endif
+  TSAN_SWITCH(B.tsan_main);
   context_switch(&f.ctx, &B.main);
 #if SIMT_ASAN
   __sanitizer_finish_switch_fiber(f.fake, &B.main_bottom, &B.main_size);
 #endif
 }
 void note_progress() { B.progress++; }
+void hb_release(const void* token) { TSAN_RELEASE(token); (void)token; }
+void hb_acquire(const void* token) { TSAN_ACQUIRE(token); (void)token; }
+void hb_fence() { TSAN_RELEASE(&B.hb_fence); TSAN_ACQUIRE(&B.hb_fence); }
 bool defer(const void* key, std::function<void()> fn) {
   if (!g_adversarial) return false;                // the caller does the work now
   g_deferred.push_back(Deferred{key, std::move(fn)});
@@ -220,19 +267,22 @@ void* dyn_smem() { return B.dyn; }
 
 void syncthreads() {
   const unsigned gen = B.bar_gen;
+  TSAN_RELEASE(&B.hb_bar);
   B.bar_arrived++; B.progress++;
   for (;;) {
-    if (B.bar_gen != gen) return;
-    if (B.bar_arrived >= B.alive) { B.bar_arrived = 0; B.bar_gen++; B.progress++; return; }   // exited threads count as arrived
+    if (B.bar_gen != gen) break;
+    if (B.bar_arrived >= B.alive) { B.bar_arrived = 0; B.bar_gen++; B.progress++; break; }   // exited threads count as arrived
     yield();
   }
+  TSAN_ACQUIRE(&B.hb_bar);
 }
 
-void warp_exchange(unsigned mask, unsigned long long v, unsigned long long out[32], unsigned* participants) {
+void warp_exchange(unsigned mask, unsigned long long v, unsigned long long out[32], unsigned* participants, bool fence) {
   const unsigned t = B.cur, lane = t & 31u, bit = 1u << lane;
   WarpSync& W = B.warp[t >> 5];
   if (!(mask & bit)) die("warp collective called by a lane that is not in its mask");
   while (W.releasing) yield();                     // the previous collective is still being picked up
+  if (fence) TSAN_RELEASE(&W.hb);
   W.val[lane] = v; W.arrived |= bit; B.progress++;
   for (;;) {
     if (W.releasing & bit) break;                  // completed by another lane
@@ -248,6 +298,7 @@ void warp_exchange(unsigned mask, unsigned long long v, unsigned long long out[3
   *participants = W.part;
   W.releasing &= ~bit; W.arrived &= ~bit;
   if (!W.releasing) B.progress++;
+  if (fence) TSAN_ACQUIRE(&W.hb);
 }
 
 void run_grid(unsigned grid, unsigned block, size_t smem, std::function<void()> body) {

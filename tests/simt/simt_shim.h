@@ -53,7 +53,14 @@ bool defer(const void* key, std::function<void()> fn);   // adversarial mode: qu
 void run_deferred(const void* key);            // run (and forget) everything queued under key
 void syncthreads();
 // Warp rendezvous: every live lane named in `mask` deposits v; each gets all deposits and who took part.
-void warp_exchange(unsigned mask, unsigned long long v, unsigned long long out[32], unsigned* participants);
+// `fence`: the rendezvous also orders the lanes' memory accesses (__syncwarp does, shuffles and ballots do not).
+void warp_exchange(unsigned mask, unsigned long long v, unsigned long long out[32], unsigned* participants, bool fence = false);
+// ThreadSanitizer build (tests/simt/build.py mode "tsan"): happens-before edges; no-ops otherwise.
+void hb_release(const void* token);
+void hb_acquire(const void* token);
+void hb_fence();                               // __threadfence: ordered against every other fibre that fences
+template <class T> inline void relaxed_store(T* p, T v) { __atomic_store_n(p, v, __ATOMIC_RELAXED); }
+template <class T> inline T relaxed_load(const T* p) { return __atomic_load_n(p, __ATOMIC_RELAXED); }
 }  // namespace simt
 #define threadIdx (simt::g.tid)
 #define blockIdx (simt::g.bid)
@@ -76,7 +83,7 @@ static inline int __ffs(unsigned v) { return __builtin_ffs((int)v); }
 static inline int __clz(int v) { return v ? __builtin_clz((unsigned)v) : 32; }
 template <class T> static inline T __ldg(const T* p) { return *p; }
 template <class T> static inline T __ldcg(const T* p) { return *p; }
-static inline void __threadfence() {}
+static inline void __threadfence() { simt::hb_fence(); }
 static inline void __nanosleep(unsigned) { simt::yield(); }
 static inline void __syncthreads() { simt::syncthreads(); }
 
@@ -90,7 +97,7 @@ inline unsigned lane_id() { return g.tid.x & 31u; }
 }  // namespace simt
 
 static inline void __syncwarp(unsigned mask = 0xFFFFFFFFu) {
-  unsigned long long o[32]; unsigned part; simt::warp_exchange(mask, 0, o, &part);
+  unsigned long long o[32]; unsigned part; simt::warp_exchange(mask, 0, o, &part, true);
 }
 template <class T> static inline T __shfl_sync(unsigned mask, T v, int src) {
   unsigned long long o[32]; unsigned part; simt::warp_exchange(mask, simt::to_bits(v), o, &part);
@@ -120,15 +127,21 @@ static inline unsigned __reduce_add_sync(unsigned mask, unsigned v) {
   return r;
 }
 
-// Atomics: one OS thread runs every fibre, and a fibre is only ever switched at a synchronisation point.
-static inline unsigned atomicAdd(unsigned* p, unsigned v) { unsigned o = *p; *p = o + v; return o; }
-static inline int atomicAdd(int* p, int v) { int o = *p; *p = o + v; return o; }
-static inline unsigned long long atomicAdd(unsigned long long* p, unsigned long long v) { unsigned long long o = *p; *p = o + v; return o; }
-static inline unsigned atomicSub(unsigned* p, unsigned v) { unsigned o = *p; *p = o - v; return o; }
-static inline int atomicSub(int* p, int v) { int o = *p; *p = o - v; return o; }
-static inline unsigned atomicMin(unsigned* p, unsigned v) { unsigned o = *p; if (v < o) *p = v; return o; }
-static inline unsigned long long atomicMin(unsigned long long* p, unsigned long long v) { unsigned long long o = *p; if (v < o) *p = v; return o; }
-static inline unsigned atomicOr(unsigned* p, unsigned v) { unsigned o = *p; *p = o | v; return o; }
+// Atomics.  One OS thread runs every fibre and a fibre is only ever switched at a synchronisation point, so plain
+// read-modify-write would do; the builtins make them atomics in the eyes of ThreadSanitizer too (relaxed, as CUDA's are).
+static inline unsigned atomicAdd(unsigned* p, unsigned v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+static inline int atomicAdd(int* p, int v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+static inline unsigned long long atomicAdd(unsigned long long* p, unsigned long long v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+static inline unsigned atomicSub(unsigned* p, unsigned v) { return __atomic_fetch_sub(p, v, __ATOMIC_RELAXED); }
+static inline int atomicSub(int* p, int v) { return __atomic_fetch_sub(p, v, __ATOMIC_RELAXED); }
+static inline unsigned atomicOr(unsigned* p, unsigned v) { return __atomic_fetch_or(p, v, __ATOMIC_RELAXED); }
+template <class T> static inline T simt_atomic_min(T* p, T v) {
+  T o = __atomic_load_n(p, __ATOMIC_RELAXED);
+  while (v < o && !__atomic_compare_exchange_n(p, &o, v, false, __ATOMIC_RELAXED, __ATOMIC_RELAXED)) {}
+  return o;
+}
+static inline unsigned atomicMin(unsigned* p, unsigned v) { return simt_atomic_min(p, v); }
+static inline unsigned long long atomicMin(unsigned long long* p, unsigned long long v) { return simt_atomic_min(p, v); }
 
 // ---------------------------------------------------------------------------------------------- runtime
 typedef int cudaError_t;

@@ -171,6 +171,25 @@ def test_kernels_under_address_and_ub_sanitizer():
     assert "SIMT-SAN OK" in r.stdout and "ERROR: AddressSanitizer" not in r.stderr and "runtime error" not in r.stderr
 
 
+def test_kernels_under_thread_sanitizer():
+    """The race check proper.  The kernels are compiled with -fsanitize=thread; every CUDA thread index is a ThreadSanitizer
+    fibre, fibre switches carry no synchronisation, and happens-before exists only where CUDA gives it: launch boundaries,
+    __syncthreads, __syncwarp (not shuffles or ballots), mbarrier arrive -> wait, __threadfence; atomics are relaxed
+    atomics.  Shared memory is reused by the next block here, so blocks are ordered one after the other (conflicts
+    between blocks are what the seeded block orders above are for).  The races the kernels have by design — K4's plain
+    prop[] stores, K5's live read of t_first, same-value clears of shared bitmap words — are relaxed atomics in this build
+    (tests/simt/build.py RACY_BY_DESIGN).  Anything else that two threads touch without such an edge is a report."""
+    lib = subprocess.run(["gcc", "-print-file-name=libtsan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(lib) or not os.path.exists(lib):
+        pytest.skip("libtsan is not installed")
+    env = dict(os.environ, LD_PRELOAD=lib, TSAN_OPTIONS="halt_on_error=0 report_signal_unsafe=0 exitcode=0")
+    env.pop("SIMT_NO_GRAPHS", None)
+    r = subprocess.run([sys.executable, os.path.join(HERE, "simt", "san_cases.py"), "tsan"], env=env, capture_output=True,
+                       text=True, timeout=1500)
+    assert r.returncode == 0 and "SIMT-SAN OK" in r.stdout, r.stdout[-2000:] + r.stderr[-3000:]
+    assert "ThreadSanitizer" not in r.stderr, r.stderr[:6000]
+
+
 def test_sanitizer_sees_an_overrun_inside_a_kernel():
     env = _asan_env()
     r = subprocess.run([sys.executable, os.path.join(HERE, "simt", "san_cases.py"), "overrun"], env=env,
