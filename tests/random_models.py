@@ -14,7 +14,7 @@ from workloads.model import (CH_BIRTH, CH_CONVERT, CH_DEGRADE, CH_DELAYED_BIRTH,
                              stack_tables)
 
 
-def random_model(seed: int, n_agents=(600, 3500), steps=(6, 12)) -> Model:
+def random_model(seed: int, n_agents=(600, 3500), steps=(6, 12), allow_big=True) -> Model:
     rng = np.random.default_rng(seed)
     pick = lambda seq: seq[int(rng.integers(len(seq)))]                                      # noqa: E731
     shape = pick(["cube", "cube", "sphere", "nucleus", "replicas"])
@@ -27,7 +27,7 @@ def random_model(seed: int, n_agents=(600, 3500), steps=(6, 12)) -> Model:
     crowd = rng.random()
     if crowd < 0.15:                                                         # one or two cells per axis: everybody is a neighbour
         size = int(rng.integers(cell // 2 + 8, 2 * cell))
-    elif crowd < 0.25:                                                       # many tiles per block: the K4 ring wraps around
+    elif crowd < 0.25 and allow_big:                                         # many tiles per block: the K4 ring wraps around
         n_agents = (8000, 16000)
     sig_hi = min(size / 7.0, 2.5 * cell)
     sigmas = [float(rng.uniform(2.0, sig_hi)) for _ in range(n_classes)]
@@ -133,5 +133,59 @@ def fuzz_parity(pkg, seeds, check_config, oracle_cls, assert_same):
             assert_same(sim, orc, f"{m.name} after {n} more steps")
         if hasattr(sim, "read_checksum"):
             assert sim.read_checksum() == orc.read_checksum(), m.name
+        ran += 1
+    return ran
+
+
+def api_sequence_parity(pkg, seeds, check_config, oracle_cls, assert_same, n_ops=14):
+    """Random sequences of API calls — step(n) with n from 0 to 19 (mixes the 8-step and 1-step graphs and both parities of
+    the ping-pong), mid-run seeding, a checkpoint written back in permuted order (sim_load_agents + t_first), per-kernel
+    profiling switched on and off (direct launches instead of graph replay) — applied to `pkg.Sim` and to the oracle
+    alike; the full state is compared after every call.  This exercises the host-side state machine of the library
+    (histogram validity, buffer parity, graph selection), not new arithmetic."""
+    ran = 0
+    for seed in seeds:
+        rng = np.random.default_rng(10_000 + seed)
+        m = random_model(seed, n_agents=(400, 1500), steps=(6, 7), allow_big=False)
+        m.counts_rows = 400
+        m.capacity *= 2
+        if check_config(m) is not None or not m.seed_records:
+            continue
+        sim, orc = pkg.Sim(m), oracle_cls(m)
+        if rng.random() < 0.7:
+            sim.seed_population(); orc.seed_population()
+        for k in range(n_ops):
+            op = rng.choice(["step", "step", "step", "seed", "reload", "profile", "checksum"])
+            if op == "step":
+                n = int(rng.choice([0, 1, 2, 3, 7, 8, 9, 16, 19]))
+                if sim.info()["step"] + n >= m.counts_rows - 1:
+                    continue
+                errs = []
+                for s in (sim, orc):
+                    try:
+                        s.step(n)
+                        errs.append(0)
+                    except RuntimeError as e:            # a population that outgrows its slots or ids: both sides must say so,
+                        errs.append(getattr(e, "code", None))     # on the same call, with the same code
+                assert errs[0] == errs[1], (m.name, k, errs)
+                if errs[0]:
+                    break
+            elif op == "seed":
+                recs = [r for r in m.seed_records if rng.random() < 0.3][:3]
+                recs = [type(r)(r.species, max(1, r.count // 10), r.replica) for r in recs]
+                place = int(rng.integers(1, 2**40))
+                sim.seed_population(recs, place_seed=place); orc.seed_population(recs, place_seed=place)
+            elif op == "reload":
+                a, info, tf = sim.read_agents(), sim.info(), sim.read_t_first()
+                perm = rng.permutation(len(a["id"]))
+                for s in (sim, orc):
+                    s.load_agents(*(a[f][perm] for f in ("x", "y", "z", "species", "id")), step=info["step"],
+                                  next_id=info["next_id"])
+                    s.load_t_first(tf)
+            elif op == "profile":
+                sim.profile_enable(bool(rng.integers(2)))
+            else:
+                assert sim.read_checksum() == orc.read_checksum(), (m.name, k)
+            assert_same(sim, orc, f"{m.name} op {k} ({op})")
         ran += 1
     return ran

@@ -150,6 +150,16 @@ def test_random_models_on_the_emulation(emu, monkeypatch):
     assert fuzz_parity(emu, range(40, 80), check_config, gp.oracle_cls(), gp.assert_same) >= 35
 
 
+def test_random_api_sequences_on_the_emulation(emu):
+    """Host-side state machine: random sequences of step(n), mid-run seeding, checkpoint reload in permuted order and
+    profiling on / off, against the oracle after every call (tests/random_models.py::api_sequence_parity).  This is the
+    kind of test that would have caught the build_graphs bug the emulation found."""
+    from paper_2606_14603_b200.binding import check_config
+    from random_models import api_sequence_parity
+
+    assert api_sequence_parity(emu, range(0, 24), check_config, gp.oracle_cls(), gp.assert_same) >= 20
+
+
 # ------------------------------------------------------------------------------------------------ sanitizers
 def _asan_env():
     lib = subprocess.run(["gcc", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()

@@ -70,3 +70,15 @@ def test_random_models_parity(gpu):
     from test_gpu_parity import assert_same, oracle_cls
 
     assert fuzz_parity(gpu, range(1000, 1060), check_config, oracle_cls(), assert_same) >= 50
+
+
+@pytest.mark.gpu
+def test_random_api_sequences_parity(gpu):
+    """Random sequences of step(n) / mid-run seeding / checkpoint reload in permuted order / per-kernel profiling on and
+    off, applied to the GPU handle and to the oracle alike, full state compared after every call: the host-side state
+    machine (histogram validity, ping-pong parity, 1-step and 8-step graphs, direct launches)."""
+    from paper_2606_14603_b200.binding import check_config
+    from random_models import api_sequence_parity
+    from test_gpu_parity import assert_same, oracle_cls
+
+    assert api_sequence_parity(gpu, range(2000, 2030), check_config, oracle_cls(), assert_same) >= 25
