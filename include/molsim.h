@@ -139,7 +139,7 @@ int sim_create(const sim_config_t* cfg, void* d_workspace, size_t workspace_byte
 int sim_seed_population(sim_t*, const sim_seed_rec_t* recs, uint32_t n_recs, uint64_t place_seed);
 
 /* Advances n_steps time steps (DESIGN.md §1 phases 1-6 per step).  All work is enqueued on the
- * stream without host synchronisation between steps (the 10 launches of a step are replayed as
+ * stream without host synchronisation between steps (the 7 launches of a step are replayed as
  * CUDA graphs captured once per handle); the call then waits for the stream once and
  * returns the sticky device error state (capacity / id space), if any.  Handles are independent:
  * several may step concurrently on different streams ("many seeds per GPU"). */
