@@ -223,7 +223,7 @@ void execute_grid(unsigned grid, unsigned block, size_t smem, const std::functio
   for (unsigned b : blocks) {
     g.bid = uint3{b, 0, 0};
     if (B.dyn) std::memset(B.dyn, 0xCD, smem);     // shared memory starts as garbage in every block
-    TSAN_RELEASE(&B.hb_launch_start);              // (again: the fill above is the host's; blocks stay unordered among themselves)
+    TSAN_RELEASE(&B.hb_launch_start);              // again: the fill above is the host's, and so is what it learnt from the block before
     run_block(block);
     // Shared memory (statics, the dynamic buffer) is reused by the next block, which on the GPU has its own: for
     // ThreadSanitizer the blocks of a launch are therefore ordered one after the other; a conflict BETWEEN blocks is
