@@ -105,6 +105,22 @@ def test_five_workload_shapes_small(emu):
     gp.run_both(emu, configs.w4(n=30_011, n_steps=17), 17, chunks=1)        # 17 = two 8-step graphs + one 1-step graph
 
 
+@pytest.mark.parametrize("case,n_rows", [("w4_4m", 3), ("w1_full", 4), ("w3_full", 12)])
+def test_full_size_oracle_traces_on_the_emulation(emu, case, n_rows):
+    """BASELINE.json's sizes on the CPU tier: the first rows of the golden oracle traces (tests/golden/trace_*.txt, written by
+    oracle/ only) — [CFG 4] at 4 M agents (the whole trace), [CFG 1] and [CFG 3] at full size — replayed by the emulated
+    kernels: state checksum, live count, next_id, t_first and the counts row of every step.  (One-off, longer prefixes,
+    [CFG 2] at full size and [CFG 4] at 64 M: profiles/r2_sanitizers.md.)"""
+    import importlib.util
+
+    spec = importlib.util.spec_from_file_location("make_traces", os.path.join(gt.GOLDEN, "make_traces.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    make = {"w4_4m": lambda: configs.w4(n=4_000_000, n_steps=2), "w1_full": lambda: configs.w1(n_steps=200),
+            "w3_full": lambda: configs.w3(**mod.W3_TRACE)}[case]
+    gt.replay(emu, make(), gt.read_trace(case)[:n_rows], case)
+
+
 def test_graph_replay_equals_direct_launches(emu, monkeypatch):
     """sim_step replays captured graphs (the emulation records and replays the launches, parameters frozen at capture as
     on the GPU); with capture refused it issues the kernels directly.  Same result, odd and even step counts, both
