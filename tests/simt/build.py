@@ -77,15 +77,17 @@ def build(sanitize=False, force: bool = False) -> str:
     common = ["g++", "-std=c++17", "-g", "-fPIC", "-DMOLSIM_CHECKS=1", "-include", os.path.join(HERE, "simt_shim.h"),
               "-I", src_dir, "-I", HERE, "-Wno-unknown-pragmas", "-Wno-attributes"]
     srcs = [os.path.join(src_dir, "molsim.cpp"), os.path.join(HERE, "simt_runtime.cpp")]
+    tmp = f"{lib}.{os.getpid()}.tmp"
     if sanitize == "tsan":      # the kernels are instrumented, the scheduler is not (it only annotates: simt_runtime.cpp)
-        objs = [os.path.join(OUT, "tsan_molsim.o"), os.path.join(OUT, "tsan_runtime.o")]
+        objs = [os.path.join(OUT, f"tsan_molsim.{os.getpid()}.o"), os.path.join(OUT, f"tsan_runtime.{os.getpid()}.o")]
         subprocess.run(common + ["-O1", "-fsanitize=thread", "-DSIMT_TSAN=1", "-c", srcs[0], "-o", objs[0]], check=True)
         subprocess.run(common + ["-O2", "-DSIMT_TSAN=1", "-c", srcs[1], "-o", objs[1]], check=True)
-        subprocess.run(["g++", "-shared", "-fsanitize=thread", "-o", lib] + objs, check=True)
+        subprocess.run(["g++", "-shared", "-fsanitize=thread", "-o", tmp] + objs, check=True)
     else:
         opt = (["-O1", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
                if sanitize else ["-O2"])
-        subprocess.run(common + opt + ["-shared", "-o", lib] + srcs, check=True)
+        subprocess.run(common + opt + ["-shared", "-o", tmp] + srcs, check=True)
+    os.replace(tmp, lib)          # a concurrent builder (pytest-xdist) never sees a half-written library
     return lib
 
 

@@ -105,7 +105,7 @@ def test_five_workload_shapes_small(emu):
     gp.run_both(emu, configs.w4(n=30_011, n_steps=17), 17, chunks=1)        # 17 = two 8-step graphs + one 1-step graph
 
 
-@pytest.mark.parametrize("case,n_rows", [("w4_4m", 3), ("w1_full", 4), ("w3_full", 12)])
+@pytest.mark.parametrize("case,n_rows", [("w4_4m", 3), ("w1_full", 3), ("w3_full", 6)])
 def test_full_size_oracle_traces_on_the_emulation(emu, case, n_rows):
     """BASELINE.json's sizes on the CPU tier: the first rows of the golden oracle traces (tests/golden/trace_*.txt, written by
     oracle/ only) — [CFG 4] at 4 M agents (the whole trace), [CFG 1] and [CFG 3] at full size — replayed by the emulated
@@ -156,14 +156,14 @@ def test_monitor_parity_small(emu):
 
 
 def test_random_models_on_the_emulation(emu, monkeypatch):
-    """Parity fuzzing (tests/random_models.py): 80 seeded random models of every shape and channel mix, the second half
+    """Parity fuzzing (tests/random_models.py): 60 seeded random models of every shape and channel mix, the second half
     under an adversarial schedule; kernels (emulated) = oracle on the full state, counts, info and checksum."""
     from paper_2606_14603_b200.binding import check_config
     from random_models import fuzz_parity
 
-    assert fuzz_parity(emu, range(0, 40), check_config, gp.oracle_cls(), gp.assert_same) >= 35
+    assert fuzz_parity(emu, range(0, 30), check_config, gp.oracle_cls(), gp.assert_same) >= 26
     monkeypatch.setenv("SIMT_SCHED_SEED", "11")
-    assert fuzz_parity(emu, range(40, 80), check_config, gp.oracle_cls(), gp.assert_same) >= 35
+    assert fuzz_parity(emu, range(30, 60), check_config, gp.oracle_cls(), gp.assert_same) >= 26
 
 
 def test_random_api_sequences_on_the_emulation(emu):
@@ -173,7 +173,7 @@ def test_random_api_sequences_on_the_emulation(emu):
     from paper_2606_14603_b200.binding import check_config
     from random_models import api_sequence_parity
 
-    assert api_sequence_parity(emu, range(0, 24), check_config, gp.oracle_cls(), gp.assert_same) >= 20
+    assert api_sequence_parity(emu, range(0, 16), check_config, gp.oracle_cls(), gp.assert_same) >= 13
 
 
 # ------------------------------------------------------------------------------------------------ sanitizers
@@ -224,7 +224,7 @@ def test_sanitizer_sees_an_overrun_inside_a_kernel():
 
 
 # ------------------------------------------------------------------------------------------------ schedules and races
-@pytest.mark.parametrize("seed", [1, 2])
+@pytest.mark.parametrize("seed", [1])
 def test_results_do_not_depend_on_the_schedule(emu, monkeypatch, seed):
     """Blocks in a random order, a random subset of the fibres in a random order on every scheduler pass, bulk copies that
     land only when somebody waits for them: the result is still the oracle's, bit for bit (every decision is keyed by id,
@@ -237,10 +237,9 @@ def test_results_do_not_depend_on_the_schedule(emu, monkeypatch, seed):
     gp.run_both(emu, configs.w3(scale=0.004, n_steps=40, cell_size=1024), 40, chunks=2)
 
 
-@pytest.mark.parametrize("name,seed", [("window_keys_without_syncwarp", 0), ("tile_read_without_full_wait", 1),
-                                       ("resolve_trusts_prop", 1)])
+@pytest.mark.parametrize("name,seed", [("window_keys_without_syncwarp", 0), ("tile_read_without_full_wait", 1)])
 def test_a_removed_synchronisation_is_noticed(name, seed):
-    """The check above has teeth (three of the five mutants of mutants.py; all five are killed, profiles/r2_sanitizers.md):
+    """The check above has teeth (two of the five mutants of mutants.py; all five are killed, profiles/r2_sanitizers.md):
     with one synchronisation taken out of the emulation's copy of the kernels (mutants.py) the
     same cases no longer match the oracle (or trip a bound check, the deadlock report, or crash)."""
     env = dict(os.environ)
