@@ -6,8 +6,8 @@ closed to the repository, so it is collected last: a failure here cannot hide an
 import numpy as np
 import pytest
 
-from workloads.model import (CH_RELEASE, SHAPE_CUBE, SHAPE_SPHERE, Channel, Compartment, Model, Reaction, SeedRecord,
-                             Species, prob_to_thr, stack_tables)
+from workloads.model import (CH_BIRTH, CH_CONVERT, CH_DEGRADE, CH_DELAYED_BIRTH, CH_RELEASE, SHAPE_CUBE, SHAPE_SPHERE,
+                             Channel, Compartment, Model, Reaction, SeedRecord, Species, prob_to_thr, stack_tables)
 
 
 @pytest.fixture(scope="module")
@@ -53,6 +53,72 @@ def body_large_gaussian_tables(gpu):
         a, b = sim.read_agents(), orc.read_agents()
         for k in ("id", "species", "x", "y", "z"):
             assert (a[k] == b[k]).all(), (m.name, k)
+
+
+def maximum_size_model():
+    """Every table at its maximum (include/molsim.h): 64 species in 8 compartments (four shells with their cores,
+    membrane twins across each), 64 reactions, 8 t_first rules with marked and delayed births, 4 channels on many species,
+    64 replicas, 255 sigma classes would not fit a test: 31 are used."""
+    rng = np.random.default_rng(64)
+    R, r_in = 150, 80
+    comps = []
+    for k in range(4):                      # four concentric shell + core pairs side by side along y
+        cy = R + k * (2 * R + 40)
+        comps += [Compartment(SHAPE_SPHERE, R, cy, R, r_out=R, r_in=r_in), Compartment(SHAPE_SPHERE, R, cy, R, r_out=r_in)]
+    n_sp, n_cls = 64, 31
+    species = [Species(f"S{i}", sigma_class=1 + i % n_cls, compartment=i % 8) for i in range(n_sp)]
+    by_comp = {c: [i for i in range(n_sp) if i % 8 == c] for c in range(8)}
+    for i in range(0, n_sp, 2):             # twins: shell species i <-> core species i + 1 of the same pair
+        species[i].cross_to, species[i].cross_thr = i + 1, prob_to_thr(0.3)
+        species[i + 1].cross_to, species[i + 1].cross_thr = i, 0xFFFFFFFF
+    reactions, seen = [], set()
+    while len(reactions) < 64:
+        c = int(rng.integers(8))
+        a, b, cx = (int(v) for v in rng.choice(by_comp[c], 3))
+        if (min(a, b), max(a, b)) in seen:
+            continue
+        seen.add((min(a, b), max(a, b)))
+        r = int(rng.integers(10, 41))
+        reactions.append(Reaction(a, b, cx, r * r, prob_to_thr(float(rng.uniform(0.2, 1.0)))))
+    reactions[0].r2 = 40 * 40
+    for rule in range(8):                   # one marked birth + one delayed birth per rule
+        s = species[rule * 8]
+        mine = by_comp[s.compartment]
+        s.channels = [Channel(CH_BIRTH, prob_to_thr(0.01), prod1=int(mine[1]), rule=rule, marks_first=True),
+                      Channel(CH_DELAYED_BIRTH, 2 + rule % 3, prod1=int(mine[2]), rule=rule),
+                      Channel(CH_RELEASE, prob_to_thr(0.02), int(mine[3]), int(mine[4])),
+                      Channel(CH_DEGRADE, prob_to_thr(0.005))]
+    for i in range(1, n_sp, 3):
+        mine = by_comp[species[i].compartment]
+        species[i].channels = [Channel(CH_CONVERT, prob_to_thr(0.02), int(mine[5])),
+                               Channel(CH_RELEASE, prob_to_thr(0.03), int(mine[6]), int(mine[7]))]
+    n_rep, shift = 64, 9                    # tile 512 >= 2 R + 1 + R_max + 1
+    recs = [SeedRecord(int(rng.integers(n_sp)), int(rng.integers(20, 60)), rep) for rep in range(n_rep) for _ in range(3)]
+    ext_y = comps[-1].cy + R + 1
+    m = Model(name="maximum_sizes", species=species, reactions=reactions, compartments=comps, table_bits=8,
+              tables=stack_tables([3.0 + 0.5 * k for k in range(n_cls)], 8), extent=(n_rep << shift, ext_y, 2 * R + 1),
+              seed=640, place_seed=641, seed_records=recs, n_steps=16, cell_size=40, n_replicas=n_rep, stride_shift=shift,
+              n_rules=8)
+    m.capacity = 4 * m.n_agents0 + 4096
+    return m.finalize()
+
+
+def body_maximum_table_sizes(gpu):
+    from paper_2606_14603_b200.binding import check_config
+    from test_gpu_parity import run_both
+
+    m = maximum_size_model()
+    assert check_config(m) is None, check_config(m)
+    assert (len(m.species), len(m.reactions), len(m.compartments), m.n_replicas, m.n_rules) == (64, 64, 8, 64, 8)
+    sim, orc = run_both(gpu, m, 16, chunks=4)
+    c = orc.read_counts()
+    assert c.shape[1:] == (64, 64) and (c[-1].sum(axis=1) > 0).all()          # every replica is populated
+    assert (orc.read_t_first() != 0xFFFFFFFF).any()                            # marked births happened
+
+
+@pytest.mark.gpu
+def test_maximum_table_sizes(gpu):
+    body_maximum_table_sizes(gpu)
 
 
 @pytest.mark.gpu
