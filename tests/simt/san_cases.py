@@ -42,7 +42,8 @@ def main():
     cases = [gp.test_tiny_dense_cube_many_events, gp.test_channel_kinds_and_priority, gp.test_crowded_single_cell,
              gt.test_homodimer_parity, gp.test_empty_population_and_mid_run_seeding, gp.test_errors,
              gt.test_load_agents_rejects_bad_positions_and_duplicate_ids, gr.test_picture_parity_nucleus_and_cytoplasm,
-             w3_shell_and_nucleus, gz.body_large_gaussian_tables, gz.body_maximum_table_sizes, random_models]
+             w3_shell_and_nucleus, gz.body_large_gaussian_tables, gz.body_maximum_table_sizes,
+             gz.body_degenerate_populations, random_models]
     import time
 
     if mode == "tsan":                 # the race check proper: the kernels that share queues, tiles and counters

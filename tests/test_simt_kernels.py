@@ -90,7 +90,7 @@ def test_rewrites_are_the_three_stated_ones():
     gt.test_homodimer_parity, gt.test_checksum_equals_oracle_and_sees_every_field,
     gt.test_w3_checkpoint_reload_with_t_first, gt.test_load_agents_rejects_bad_positions_and_duplicate_ids,
     gr.test_picture_parity_nucleus_and_cytoplasm, gr.test_compiled_compartmentalised_model_parity,
-    gz.body_large_gaussian_tables, gz.body_maximum_table_sizes,
+    gz.body_large_gaussian_tables, gz.body_maximum_table_sizes, gz.body_degenerate_populations,
 ], ids=lambda f: f.__name__)
 def test_gpu_test_body_on_the_emulation(emu, body):
     body(emu)

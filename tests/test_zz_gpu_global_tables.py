@@ -148,3 +148,28 @@ def test_random_api_sequences_parity(gpu):
     from test_gpu_parity import assert_same, oracle_cls
 
     assert api_sequence_parity(gpu, range(2000, 2030), check_config, oracle_cls(), assert_same) >= 25
+
+
+def body_degenerate_populations(gpu):
+    """Degenerate populations: exactly `capacity` agents (the last tile of every pass ends at the last slot, K4's bulk
+    copies and group reads run into the slack behind it), a population in which everybody degrades in the first step
+    (stepping goes on with nobody alive), and a single agent."""
+    from test_gpu_parity import run_both, tiny_cube
+
+    m = tiny_cube(L=300, n_a=1024, n_b=1024, p_bind=0.6, p_rel=0.0, cell=64)       # no release: the population only shrinks
+    m.capacity = 2048
+    run_both(gpu, m, 6, chunks=2)
+    X = 0
+    m = Model(name="all_degrade", species=[Species("X", 1, channels=[Channel(CH_DEGRADE, 0xFFFFFFFF)])], reactions=[],
+              compartments=[Compartment(SHAPE_CUBE, L=500)], table_bits=10, tables=stack_tables([30.0], 10),
+              extent=(500,) * 3, seed=5, place_seed=6, seed_records=[SeedRecord(X, 3000)], n_steps=5, cell_size=50).finalize()
+    sim, orc = run_both(gpu, m, 5, chunks=5)
+    assert sim.info()["n_live"] == 0 and sim.read_counts()[1:].sum() == 0
+    m = tiny_cube(L=300, n_a=1, n_b=0, cell=64)
+    m.seed_records = [r for r in m.seed_records if r.count]
+    run_both(gpu, m, 9, chunks=3)
+
+
+@pytest.mark.gpu
+def test_degenerate_populations(gpu):
+    body_degenerate_populations(gpu)
