@@ -7,7 +7,9 @@
 //   * the kernels' logic is checked against the oracle by `pytest -m "not gpu"`, on a machine without a GPU;
 //   * the same build under -fsanitize=address,undefined is a memcheck of every kernel access against the exact
 //     workspace allocation (compute-sanitizer is closed on the GPU pool, profiles/r2_sanitizers.md);
-//   * the workspace is filled with garbage before use, so reliance on zero-initialised memory shows up as a mismatch.
+//   * the workspace is filled with garbage before use, so reliance on zero-initialised memory shows up as a mismatch;
+//   * seeded adversarial schedules (SIMT_SCHED_SEED) and a ThreadSanitizer build (one TSan fibre per CUDA thread,
+//     happens-before only where CUDA gives it) are the race check.
 // What it is NOT: a CPU fallback.  The package (paper_2606_14603_b200/) never builds, loads or mentions it; the
 // product path fails loudly without the CUDA library (binding.load_library).  It says nothing about performance.
 #pragma once
