@@ -54,7 +54,9 @@ inline void fence_proxy_async() {}
 EMU_BAR inline void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
   if (((uintptr_t)dst | (uintptr_t)src | bytes) & 15u) emu_fail("bulk copy operands must be 16-byte aligned multiples of 16");
   auto land = [=]() EMU_BAR {
-    std::memcpy(dst, src, bytes);          // the async proxy's write, done by whichever fibre lands the copy
+    simt::hb_acquire(bar);                 // the copy was issued after the issuer's expect_tx on this barrier: a late landing
+                                           // (seeded schedules: done by whichever fibre polls first) keeps that order
+    std::memcpy(dst, src, bytes);          // the async proxy's write
     simt::hb_release(bar);
     EmuMbar* m = emu_bar(bar);
     m->tx -= (int32_t)bytes;

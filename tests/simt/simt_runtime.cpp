@@ -255,9 +255,11 @@ void hb_fence() { TSAN_RELEASE(&B.hb_fence); TSAN_ACQUIRE(&B.hb_fence); }
 bool defer(const void* key, std::function<void()> fn) {
   if (!g_adversarial) return false;                // the caller does the work now
   g_deferred.push_back(Deferred{key, std::move(fn)});
+  TSAN_RELEASE(key);                                // whoever runs it later comes after the issue (and its allocation)
   return true;
 }
 void run_deferred(const void* key) {
+  TSAN_ACQUIRE(key);
   for (size_t k = 0; k < g_deferred.size();) {
     if (g_deferred[k].key == key) { auto fn = std::move(g_deferred[k].fn); g_deferred.erase(g_deferred.begin() + k); fn(); }
     else ++k;
